@@ -1,0 +1,129 @@
+/* scalingattn.h -- C ABI of libscalingattn.so: the B200 (sm_100a) hot path of ScalingAttention,
+ * the bit-wise block-sparse attention forward pass the paper calls the "crm kernel".
+ *
+ * Citations are line numbers of the paper text /root/reference/PAPER.md.
+ *
+ * Conventions (all entry points):
+ *  - Pointers are DEVICE pointers unless the parameter name ends in _host. The caller owns every
+ *    buffer; the library never frees or retains a caller pointer past the stream-ordered end of
+ *    the call, and never allocates device memory (scratch comes in as `workspace`; the short
+ *    sa_block_sparse_attn_fwd keeps one lazily grown internal workspace per process instead).
+ *  - `stream` is a cudaStream_t passed as void*. Calls enqueue work on it and return without
+ *    synchronising; outputs are valid once the stream reaches the end of the enqueued work.
+ *  - Errors are return codes; nothing is launched when validation fails; sa_last_error() holds a
+ *    thread-local detail string for the last non-OK status. No exceptions, no abort.
+ *  - Results are deterministic: each (batch, head, query block) is reduced by one CTA over its
+ *    active key blocks in ascending order; no atomics touch out or lse.
+ *  - Supported shapes: (D, Bq, Bk) in {(128,128,128), (64,64,64)}. Anything else is
+ *    SA_ERR_UNSUPPORTED, never a silent slow path. The device must be compute capability 10.x.
+ *
+ * Compressed Row Mask (CRM) layout (Sec. 4.3.2; bit order from Alg. 2,
+ * INDEX = base + CTZ(val), base += 32 per word):
+ *    mask_bits: uint32 [H][NQB][W], NQB = N/Bq, NKB = N/Bk, W = ceil(NKB/32);
+ *    key block v of query block u of head h is active  <=>  bit (v % 32) of word (v / 32) of row
+ *    (h, u) is 1. Bits at positions >= NKB are ignored by the forward pass and written as 0 by
+ *    sa_pack_mask. The mask is per head and shared across the batch.
+ */
+#ifndef SCALINGATTN_H_
+#define SCALINGATTN_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define SA_API __attribute__((visibility("default")))
+#else
+#define SA_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  SA_OK = 0,
+  SA_ERR_INVALID_ARG = 1, /* null pointer, non-positive size, N % Bq/Bk != 0, n_valid outside [1,N],
+                             misaligned pointer (16 B), bad variant id */
+  SA_ERR_UNSUPPORTED = 2, /* (D,Bq,Bk) outside the supported set, or not an sm_100 device */
+  SA_ERR_CUDA = 3,        /* a CUDA runtime / driver call failed; text in sa_last_error() */
+  SA_ERR_WORKSPACE = 4    /* workspace null or smaller than the *_workspace_bytes() figure */
+} sa_status;
+
+/* Words per CRM bit-row = ceil((N/Bk)/32) (256k tokens, 128-blocks -> 64 words).
+ * Host helper, no CUDA call. Returns -1 for non-positive arguments or N % Bk != 0. */
+SA_API int sa_mask_words_per_row(int N, int Bk);
+
+/* Bytes of device scratch the calls below need. Host helpers, no CUDA call; 0 on bad arguments. */
+SA_API size_t sa_pack_mask_workspace_bytes(int H, int NQB, int NKB);
+SA_API size_t sa_fwd_workspace_bytes(int B, int H, int N, int Bq);
+/* Device staging a sa_block_sparse_attn_fwd_host call needs (q,k,v,out,lse,mask + fwd workspace). */
+SA_API size_t sa_fwd_host_scratch_bytes(int B, int H, int N, int D, int Bq, int Bk);
+
+/* Mask instantiation (PAPER.md:103 M_p = 1(T <= p); Alg. 1 l.31 PAPER.md:437) in the form
+ * "per-head top-fraction of block scores -> packed bits" (readings P1-P4):
+ *   scores  : fp32 [H][NQB][NKB] row-major, finite (NaN sorts lowest; -0 == +0)
+ *   density : fp32 [H]; head h keeps k_h = clamp(floor((double)density[h]*NQB*NKB + 0.5), 1, NQB*NKB)
+ *             blocks, taken in (score descending, flat index u*NKB+v ascending) order
+ *   force_diag != 0: bits (u,u) are forced on, rank first and count towards k_h (k_h is raised
+ *             to min(NQB,NKB) if smaller)
+ *   mask_bits (out): uint32 [H][NQB][W]; exactly k_h bits set per head.
+ * Bit-exact and deterministic. workspace >= sa_pack_mask_workspace_bytes(H,NQB,NKB), 16 B aligned. */
+SA_API sa_status sa_pack_mask(const float* scores, const float* density, uint32_t* mask_bits, int H,
+                       int NQB, int NKB, int force_diag, void* workspace, size_t workspace_bytes,
+                       void* stream);
+
+/* Block-sparse attention forward (Sec. 4.3.2; Alg. 2):
+ *   out[b,h,i,:] = sum_j softmax_j(scale * <q[b,h,i,:], k[b,h,j,:]>) * v[b,h,j,:]
+ *   lse[b,h,i]   = ln sum_j exp(scale * <q_i, k_j>)                       (natural log)
+ * with j ranging over the tokens of the key blocks whose bit is set in row (h, i / Bq). Masked key
+ * blocks are never loaded and never multiplied. A row with no active key gives out = 0, lse = -inf.
+ *   q, k, v, out : bf16 [B][H][N][D] contiguous, 16 B aligned;  lse : fp32 [B][H][N]
+ *   scale        : softmax scale (e.g. 1/sqrt(D)); arithmetic is bf16 x bf16 -> fp32.
+ * All N tokens are real. Uses an internal workspace (grown with cudaMalloc on first use / when a
+ * larger problem arrives, which synchronises; freed at process exit). */
+SA_API sa_status sa_block_sparse_attn_fwd(const void* q, const void* k, const void* v,
+                                   const uint32_t* mask_bits, void* out, float* lse, int B, int H,
+                                   int N, int D, int Bq, int Bk, float scale, void* stream);
+
+/* Same, plus n_valid (keys >= n_valid get exactly zero weight, even inside an active block; query
+ * rows >= n_valid are computed like any other row) and a caller-provided workspace of at least
+ * sa_fwd_workspace_bytes(B,H,N,Bq) bytes (16 B aligned), so nothing is allocated in the call. */
+SA_API sa_status sa_block_sparse_attn_fwd_ex(const void* q, const void* k, const void* v,
+                                      const uint32_t* mask_bits, void* out, float* lse, int B,
+                                      int H, int N, int n_valid, int D, int Bq, int Bk,
+                                      float scale, void* workspace, size_t workspace_bytes,
+                                      void* stream);
+
+/* End-to-end form with HOST buffers (pinned memory recommended): copies q, k, v and the mask to
+ * `scratch` (device, >= sa_fwd_host_scratch_bytes, 256 B aligned), runs the forward pass there and
+ * copies out and lse back, all on `stream`, without synchronising. */
+SA_API sa_status sa_block_sparse_attn_fwd_host(const void* q_host, const void* k_host, const void* v_host,
+                                        const uint32_t* mask_bits_host, void* out_host,
+                                        float* lse_host, int B, int H, int N, int n_valid, int D,
+                                        int Bq, int Bk, float scale, void* scratch,
+                                        size_t scratch_bytes, void* stream);
+
+/* CRM forward iterator on the device (Alg. 2), exposed so that its walk can be
+ * checked on its own: for every row (h,u) writes the active key blocks in the order the iterator
+ * yields them to idx[h][u][0..cnt) (int32 [H][NQB][NKB]) and their number to cnt[h][u]
+ * (int32 [H][NQB]). Entries of idx past cnt are left untouched. */
+SA_API sa_status sa_enumerate_active_blocks(const uint32_t* mask_bits, int H, int NQB, int NKB,
+                                     int32_t* idx, int32_t* cnt, void* stream);
+
+/* Which CUDA kernel the forward pass uses. 0 (default): automatic -- the tcgen05/TMEM/TMA kernel
+ * for (128,128,128), the mma.sync kernel for (64,64,64). 1: the mma.sync kernel for every
+ * supported shape (a second CUDA implementation kept for cross-checking; not a fallback: it is
+ * never chosen implicitly for a shape the fast kernel supports). Process-wide. */
+SA_API sa_status sa_set_fwd_variant(int variant);
+SA_API int sa_get_fwd_variant(void);
+
+/* Number of kernels the last forward call on this thread enqueued (for bench accounting). */
+SA_API int sa_last_launch_count(void);
+
+SA_API const char* sa_status_string(sa_status s); /* static string, never freed */
+SA_API const char* sa_last_error(void);           /* thread-local text for the last non-OK status */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SCALINGATTN_H_ */

@@ -1,0 +1,216 @@
+"""Thin ctypes binding over libscalingattn.so (include/scalingattn.h), same names as the C ABI.
+
+Argument marshalling only: every step of the hot path runs in the CUDA kernels of the library.
+torch is used for device memory and streams. There is no CPU fallback: if the library cannot be
+loaded, or a call returns a non-OK status, SAError is raised.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libscalingattn.so")
+_lib = None
+
+SA_OK = 0
+
+
+class SAError(RuntimeError):
+    def __init__(self, status: int, name: str, detail: str):
+        super().__init__(f"{name} ({status}): {detail}")
+        self.status = status
+        self.name = name
+        self.detail = detail
+
+
+def library_path() -> str:
+    return _LIB_PATH
+
+
+def load_library() -> C.CDLL:
+    """dlopen the in-tree library; fails loudly if it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise SAError(-1, "SA_ERR_NOT_BUILT",
+                      f"{_LIB_PATH} missing: run `python -m paper_2606_23019_b200.build` "
+                      "(there is no CPU fallback)")
+    lib = C.CDLL(_LIB_PATH)
+    vp, ip, fp, sz = C.c_void_p, C.c_int, C.c_float, C.c_size_t
+    lib.sa_mask_words_per_row.restype = ip
+    lib.sa_mask_words_per_row.argtypes = [ip, ip]
+    lib.sa_pack_mask_workspace_bytes.restype = sz
+    lib.sa_pack_mask_workspace_bytes.argtypes = [ip, ip, ip]
+    lib.sa_fwd_workspace_bytes.restype = sz
+    lib.sa_fwd_workspace_bytes.argtypes = [ip, ip, ip, ip]
+    lib.sa_fwd_host_scratch_bytes.restype = sz
+    lib.sa_fwd_host_scratch_bytes.argtypes = [ip] * 6
+    lib.sa_pack_mask.restype = ip
+    lib.sa_pack_mask.argtypes = [vp, vp, vp, ip, ip, ip, ip, vp, sz, vp]
+    lib.sa_block_sparse_attn_fwd.restype = ip
+    lib.sa_block_sparse_attn_fwd.argtypes = [vp, vp, vp, vp, vp, vp, ip, ip, ip, ip, ip, ip, fp, vp]
+    lib.sa_block_sparse_attn_fwd_ex.restype = ip
+    lib.sa_block_sparse_attn_fwd_ex.argtypes = [vp, vp, vp, vp, vp, vp, ip, ip, ip, ip, ip, ip, ip,
+                                                fp, vp, sz, vp]
+    lib.sa_block_sparse_attn_fwd_host.restype = ip
+    lib.sa_block_sparse_attn_fwd_host.argtypes = [vp, vp, vp, vp, vp, vp, ip, ip, ip, ip, ip, ip,
+                                                  ip, fp, vp, sz, vp]
+    lib.sa_enumerate_active_blocks.restype = ip
+    lib.sa_enumerate_active_blocks.argtypes = [vp, ip, ip, ip, vp, vp, vp]
+    lib.sa_set_fwd_variant.restype = ip
+    lib.sa_set_fwd_variant.argtypes = [ip]
+    lib.sa_get_fwd_variant.restype = ip
+    lib.sa_last_launch_count.restype = ip
+    lib.sa_status_string.restype = C.c_char_p
+    lib.sa_status_string.argtypes = [ip]
+    lib.sa_last_error.restype = C.c_char_p
+    _lib = lib
+    return lib
+
+
+def _check(status: int) -> None:
+    if status != SA_OK:
+        lib = load_library()
+        raise SAError(status, lib.sa_status_string(status).decode(), lib.sa_last_error().decode())
+
+
+def _ptr(t) -> int:
+    return 0 if t is None else t.data_ptr()
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
+
+
+def sa_status_string(status: int) -> str:
+    return load_library().sa_status_string(status).decode()
+
+
+def sa_last_error() -> str:
+    return load_library().sa_last_error().decode()
+
+
+def sa_mask_words_per_row(N: int, Bk: int) -> int:
+    return load_library().sa_mask_words_per_row(N, Bk)
+
+
+def sa_pack_mask_workspace_bytes(H: int, NQB: int, NKB: int) -> int:
+    return load_library().sa_pack_mask_workspace_bytes(H, NQB, NKB)
+
+
+def sa_fwd_workspace_bytes(B: int, H: int, N: int, Bq: int) -> int:
+    return load_library().sa_fwd_workspace_bytes(B, H, N, Bq)
+
+
+def sa_fwd_host_scratch_bytes(B: int, H: int, N: int, D: int, Bq: int, Bk: int) -> int:
+    return load_library().sa_fwd_host_scratch_bytes(B, H, N, D, Bq, Bk)
+
+
+def sa_set_fwd_variant(variant: int) -> None:
+    _check(load_library().sa_set_fwd_variant(variant))
+
+
+def sa_get_fwd_variant() -> int:
+    return load_library().sa_get_fwd_variant()
+
+
+def sa_last_launch_count() -> int:
+    return load_library().sa_last_launch_count()
+
+
+def sa_pack_mask(scores, density, force_diag: bool = True, mask_bits=None, workspace=None,
+                 stream=None):
+    """scores fp32 [H][NQB][NKB], density fp32 [H] (device) -> mask_bits int32 [H][NQB][W]
+    (uint32 bit patterns; torch has no general uint32 support, so the storage dtype is int32)."""
+    lib = load_library()
+    assert scores.dtype == torch.float32 and scores.is_contiguous() and scores.dim() == 3
+    assert density.dtype == torch.float32 and density.is_contiguous()
+    H, NQB, NKB = scores.shape
+    assert density.shape == (H,)
+    W = (NKB + 31) // 32
+    if mask_bits is None:
+        mask_bits = torch.empty((H, NQB, W), dtype=torch.int32, device=scores.device)
+    need = lib.sa_pack_mask_workspace_bytes(H, NQB, NKB)
+    if workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=scores.device)
+    _check(lib.sa_pack_mask(_ptr(scores), _ptr(density), _ptr(mask_bits), H, NQB, NKB,
+                            int(bool(force_diag)), _ptr(workspace), workspace.numel(),
+                            _stream(stream)))
+    return mask_bits
+
+
+def _fwd_shapes(q, k, v, mask_bits, Bq, Bk):
+    assert q.dtype == k.dtype == v.dtype == torch.bfloat16
+    assert q.is_contiguous() and k.is_contiguous() and v.is_contiguous()
+    assert q.shape == k.shape == v.shape and q.dim() == 4
+    B, H, N, D = q.shape
+    assert mask_bits.dtype == torch.int32 and mask_bits.is_contiguous()
+    if N % Bq == 0 and N % Bk == 0:
+        assert tuple(mask_bits.shape) == (H, N // Bq, (N // Bk + 31) // 32), mask_bits.shape
+    return B, H, N, D
+
+
+def sa_block_sparse_attn_fwd(q, k, v, mask_bits, Bq: int, Bk: int, scale: float, out=None,
+                             lse=None, stream=None):
+    """The signature BASELINE.json names (internal workspace, all N tokens real)."""
+    lib = load_library()
+    B, H, N, D = _fwd_shapes(q, k, v, mask_bits, Bq, Bk)
+    if out is None:
+        out = torch.empty_like(q)
+    if lse is None:
+        lse = torch.empty((B, H, N), dtype=torch.float32, device=q.device)
+    _check(lib.sa_block_sparse_attn_fwd(_ptr(q), _ptr(k), _ptr(v), _ptr(mask_bits), _ptr(out),
+                                        _ptr(lse), B, H, N, D, Bq, Bk, float(scale),
+                                        _stream(stream)))
+    return out, lse
+
+
+def sa_block_sparse_attn_fwd_ex(q, k, v, mask_bits, Bq: int, Bk: int, scale: float,
+                                n_valid=None, out=None, lse=None, workspace=None, stream=None):
+    lib = load_library()
+    B, H, N, D = _fwd_shapes(q, k, v, mask_bits, Bq, Bk)
+    n_valid = N if n_valid is None else int(n_valid)
+    if out is None:
+        out = torch.empty_like(q)
+    if lse is None:
+        lse = torch.empty((B, H, N), dtype=torch.float32, device=q.device)
+    if workspace is None:
+        workspace = torch.empty(max(lib.sa_fwd_workspace_bytes(B, H, N, Bq), 256),
+                                dtype=torch.uint8, device=q.device)
+    _check(lib.sa_block_sparse_attn_fwd_ex(_ptr(q), _ptr(k), _ptr(v), _ptr(mask_bits), _ptr(out),
+                                           _ptr(lse), B, H, N, n_valid, D, Bq, Bk, float(scale),
+                                           _ptr(workspace), workspace.numel(), _stream(stream)))
+    return out, lse
+
+
+def sa_block_sparse_attn_fwd_host(q, k, v, mask_bits, out, lse, Bq: int, Bk: int, scale: float,
+                                  n_valid, scratch, stream=None):
+    """End-to-end form: q, k, v, mask_bits, out, lse are HOST (pinned) tensors, scratch is device."""
+    lib = load_library()
+    B, H, N, D = _fwd_shapes(q, k, v, mask_bits, Bq, Bk)
+    for t in (q, k, v, mask_bits, out, lse):
+        assert t.device.type == "cpu"
+    assert out.dtype == torch.bfloat16 and out.shape == q.shape and out.is_contiguous()
+    assert lse.dtype == torch.float32 and tuple(lse.shape) == (B, H, N) and lse.is_contiguous()
+    _check(lib.sa_block_sparse_attn_fwd_host(_ptr(q), _ptr(k), _ptr(v), _ptr(mask_bits), _ptr(out),
+                                             _ptr(lse), B, H, N, int(n_valid), D, Bq, Bk,
+                                             float(scale), _ptr(scratch), scratch.numel(),
+                                             _stream(stream)))
+    return out, lse
+
+
+def sa_enumerate_active_blocks(mask_bits, NKB: int, stream=None):
+    lib = load_library()
+    H, NQB, W = mask_bits.shape
+    assert mask_bits.dtype == torch.int32 and mask_bits.is_contiguous()
+    idx = torch.full((H, NQB, NKB), -1, dtype=torch.int32, device=mask_bits.device)
+    cnt = torch.zeros((H, NQB), dtype=torch.int32, device=mask_bits.device)
+    _check(lib.sa_enumerate_active_blocks(_ptr(mask_bits), H, NQB, NKB, _ptr(idx), _ptr(cnt),
+                                          _stream(stream)))
+    return idx, cnt

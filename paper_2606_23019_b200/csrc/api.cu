@@ -1,0 +1,285 @@
+// api.cu -- the C ABI of libscalingattn.so (include/scalingattn.h): argument validation, error
+// reporting, workspace carving and kernel dispatch. No arithmetic of the method lives here.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+
+#include "common.cuh"
+
+namespace {
+
+thread_local char g_err[512] = "";
+thread_local int g_last_launches = 0;
+int g_variant = 0;
+
+sa_status fail(sa_status s, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof g_err, fmt, ap);
+  va_end(ap);
+  return s;
+}
+
+sa_status cuda_fail(cudaError_t e, const char* what) {
+  return fail(SA_ERR_CUDA, "%s: %s (%s)", what, cudaGetErrorString(e), cudaGetErrorName(e));
+}
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+constexpr int kMaxBlocksPerRow = 12288;  // shared-memory bound of the schedule pre-pass
+constexpr int kMaxGroups = 8192;         // B*H bound of the schedule pre-pass
+
+// compute capability of the current device must be 10.x (sm_100a binary)
+sa_status check_device() {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
+  static std::mutex mu;
+  static int cached_dev = -1, cached_major = 0;
+  std::lock_guard<std::mutex> lk(mu);
+  if (cached_dev != dev) {
+    int major = 0;
+    e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaDeviceGetAttribute");
+    cached_dev = dev;
+    cached_major = major;
+  }
+  if (cached_major != 10)
+    return fail(SA_ERR_UNSUPPORTED, "device compute capability %d.x; this library is sm_100a only",
+                cached_major);
+  return SA_OK;
+}
+
+sa_status validate_shape(int B, int H, int N, int n_valid, int D, int Bq, int Bk, float scale) {
+  if (B <= 0 || H <= 0 || N <= 0 || D <= 0 || Bq <= 0 || Bk <= 0)
+    return fail(SA_ERR_INVALID_ARG, "sizes must be positive (B=%d H=%d N=%d D=%d Bq=%d Bk=%d)", B,
+                H, N, D, Bq, Bk);
+  if (!((D == 128 && Bq == 128 && Bk == 128) || (D == 64 && Bq == 64 && Bk == 64)))
+    return fail(SA_ERR_UNSUPPORTED,
+                "(D,Bq,Bk)=(%d,%d,%d) unsupported; supported: (128,128,128), (64,64,64)", D, Bq, Bk);
+  if (N % Bq != 0 || N % Bk != 0)
+    return fail(SA_ERR_INVALID_ARG, "N=%d must be a multiple of Bq=%d and Bk=%d", N, Bq, Bk);
+  if (n_valid < 1 || n_valid > N)
+    return fail(SA_ERR_INVALID_ARG, "n_valid=%d outside [1, N=%d]", n_valid, N);
+  if (!(scale > 0.f) || !(scale < 3.0e38f))
+    return fail(SA_ERR_INVALID_ARG, "scale must be finite and positive");
+  if (N / Bq > kMaxBlocksPerRow || static_cast<long long>(B) * H > kMaxGroups)
+    return fail(SA_ERR_UNSUPPORTED, "N/Bq=%d > %d or B*H=%lld > %d", N / Bq, kMaxBlocksPerRow,
+                static_cast<long long>(B) * H, kMaxGroups);
+  return SA_OK;
+}
+
+// internal workspace of the short-signature call
+std::mutex g_ws_mu;
+void* g_ws = nullptr;
+size_t g_ws_bytes = 0;
+struct WsFree {
+  ~WsFree() {
+    if (g_ws) cudaFree(g_ws);
+  }
+} g_ws_free;
+
+}  // namespace
+
+extern "C" {
+
+int sa_mask_words_per_row(int N, int Bk) {
+  if (N <= 0 || Bk <= 0 || N % Bk != 0) return -1;
+  return (N / Bk + 31) / 32;
+}
+
+size_t sa_pack_mask_workspace_bytes(int H, int NQB, int NKB) {
+  if (H <= 0 || NQB <= 0 || NKB <= 0) return 0;
+  return sa::pack_mask_workspace_bytes(H, NQB, NKB);
+}
+
+size_t sa_fwd_workspace_bytes(int B, int H, int N, int Bq) {
+  if (B <= 0 || H <= 0 || N <= 0 || Bq <= 0 || N % Bq != 0) return 0;
+  return sa::fwd_workspace_bytes(B, H, N / Bq);
+}
+
+static size_t al256(size_t x) { return (x + 255) / 256 * 256; }
+
+size_t sa_fwd_host_scratch_bytes(int B, int H, int N, int D, int Bq, int Bk) {
+  if (B <= 0 || H <= 0 || N <= 0 || D <= 0 || Bq <= 0 || Bk <= 0 || N % Bq || N % Bk) return 0;
+  const size_t t = al256(static_cast<size_t>(B) * H * N * D * 2);
+  const size_t l = al256(static_cast<size_t>(B) * H * N * 4);
+  const size_t m = al256(static_cast<size_t>(H) * (N / Bq) * ((N / Bk + 31) / 32) * 4);
+  return 4 * t + l + m + sa_fwd_workspace_bytes(B, H, N, Bq);
+}
+
+sa_status sa_pack_mask(const float* scores, const float* density, uint32_t* mask_bits, int H,
+                       int NQB, int NKB, int force_diag, void* workspace, size_t workspace_bytes,
+                       void* stream) {
+  if (!scores || !density || !mask_bits)
+    return fail(SA_ERR_INVALID_ARG, "sa_pack_mask: null pointer");
+  if (H <= 0 || NQB <= 0 || NKB <= 0)
+    return fail(SA_ERR_INVALID_ARG, "sa_pack_mask: sizes must be positive (H=%d NQB=%d NKB=%d)", H,
+                NQB, NKB);
+  if (static_cast<long long>(NQB) * NKB > 0x7FFFFFFFLL)
+    return fail(SA_ERR_UNSUPPORTED, "sa_pack_mask: NQB*NKB exceeds 2^31-1");
+  if (!aligned16(scores) || !aligned16(mask_bits) || !aligned16(workspace))
+    return fail(SA_ERR_INVALID_ARG, "sa_pack_mask: pointers must be 16-byte aligned");
+  const size_t need = sa::pack_mask_workspace_bytes(H, NQB, NKB);
+  if (!workspace || workspace_bytes < need)
+    return fail(SA_ERR_WORKSPACE, "sa_pack_mask: workspace %zu B < %zu B", workspace_bytes, need);
+  sa_status s = check_device();
+  if (s != SA_OK) return s;
+  cudaError_t e = sa::launch_pack_mask(scores, density, mask_bits, H, NQB, NKB, force_diag ? 1 : 0,
+                                       workspace, static_cast<cudaStream_t>(stream));
+  if (e != cudaSuccess) return cuda_fail(e, "sa_pack_mask launch");
+  return SA_OK;
+}
+
+sa_status sa_block_sparse_attn_fwd_ex(const void* q, const void* k, const void* v,
+                                      const uint32_t* mask_bits, void* out, float* lse, int B,
+                                      int H, int N, int n_valid, int D, int Bq, int Bk,
+                                      float scale, void* workspace, size_t workspace_bytes,
+                                      void* stream) {
+  g_last_launches = 0;
+  if (!q || !k || !v || !mask_bits || !out || !lse)
+    return fail(SA_ERR_INVALID_ARG, "sa_block_sparse_attn_fwd: null pointer");
+  sa_status s = validate_shape(B, H, N, n_valid, D, Bq, Bk, scale);
+  if (s != SA_OK) return s;
+  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out) || !aligned16(mask_bits) ||
+      !aligned16(lse) || !aligned16(workspace))
+    return fail(SA_ERR_INVALID_ARG, "sa_block_sparse_attn_fwd: pointers must be 16-byte aligned");
+  const size_t need = sa::fwd_workspace_bytes(B, H, N / Bq);
+  if (!workspace || workspace_bytes < need)
+    return fail(SA_ERR_WORKSPACE, "sa_block_sparse_attn_fwd: workspace %zu B < %zu B",
+                workspace_bytes, need);
+  s = check_device();
+  if (s != SA_OK) return s;
+
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  sa::FwdParams p;
+  p.q = static_cast<const __nv_bfloat16*>(q);
+  p.k = static_cast<const __nv_bfloat16*>(k);
+  p.v = static_cast<const __nv_bfloat16*>(v);
+  p.mask_bits = mask_bits;
+  p.out = static_cast<__nv_bfloat16*>(out);
+  p.lse = lse;
+  p.B = B; p.H = H; p.N = N; p.n_valid = n_valid; p.D = D; p.Bq = Bq; p.Bk = Bk;
+  p.NQB = N / Bq; p.NKB = N / Bk; p.W = (p.NKB + 31) / 32;
+  p.scale = scale;
+  p.scale_log2 = scale * 1.4426950408889634f;
+  const sa::FwdWorkspace w = sa::carve_fwd_workspace(workspace, B, H, p.NQB);
+  p.unit_order = w.unit_order;
+  p.counter = w.cursor;
+
+  const bool fast = (g_variant == 0 && D == 128);
+  const int rows_per_item = fast ? 2 : 1;
+  p.n_items = B * H * ((p.NQB + rows_per_item - 1) / rows_per_item);
+  cudaError_t e = sa::launch_schedule(p, w, rows_per_item, st, &g_last_launches);
+  if (e != cudaSuccess) return cuda_fail(e, "schedule pre-pass launch");
+  if (fast) {
+    const char* txt = nullptr;
+    e = sa::launch_fwd_tcgen05(p, nullptr, st, &g_last_launches, &txt);
+    if (e != cudaSuccess) return cuda_fail(e, txt ? txt : "tcgen05 forward launch");
+  } else {
+    e = sa::launch_fwd_mma_sync(p, st, &g_last_launches);
+    if (e != cudaSuccess) return cuda_fail(e, "mma.sync forward launch");
+  }
+  return SA_OK;
+}
+
+sa_status sa_block_sparse_attn_fwd(const void* q, const void* k, const void* v,
+                                   const uint32_t* mask_bits, void* out, float* lse, int B, int H,
+                                   int N, int D, int Bq, int Bk, float scale, void* stream) {
+  const size_t need = sa_fwd_workspace_bytes(B, H, N, Bq);
+  if (need == 0) return fail(SA_ERR_INVALID_ARG, "sa_block_sparse_attn_fwd: bad sizes");
+  void* ws = nullptr;
+  {
+    std::lock_guard<std::mutex> lk(g_ws_mu);
+    if (g_ws_bytes < need) {
+      if (g_ws) {
+        cudaDeviceSynchronize();
+        cudaFree(g_ws);
+        g_ws = nullptr;
+        g_ws_bytes = 0;
+      }
+      cudaError_t e = cudaMalloc(&g_ws, need);
+      if (e != cudaSuccess) return cuda_fail(e, "cudaMalloc(internal workspace)");
+      g_ws_bytes = need;
+    }
+    ws = g_ws;
+  }
+  return sa_block_sparse_attn_fwd_ex(q, k, v, mask_bits, out, lse, B, H, N, N, D, Bq, Bk, scale,
+                                     ws, need, stream);
+}
+
+sa_status sa_block_sparse_attn_fwd_host(const void* q_host, const void* k_host, const void* v_host,
+                                        const uint32_t* mask_bits_host, void* out_host,
+                                        float* lse_host, int B, int H, int N, int n_valid, int D,
+                                        int Bq, int Bk, float scale, void* scratch,
+                                        size_t scratch_bytes, void* stream) {
+  if (!q_host || !k_host || !v_host || !mask_bits_host || !out_host || !lse_host)
+    return fail(SA_ERR_INVALID_ARG, "sa_block_sparse_attn_fwd_host: null pointer");
+  sa_status s = validate_shape(B, H, N, n_valid, D, Bq, Bk, scale);
+  if (s != SA_OK) return s;
+  const size_t need = sa_fwd_host_scratch_bytes(B, H, N, D, Bq, Bk);
+  if (!scratch || scratch_bytes < need || (reinterpret_cast<uintptr_t>(scratch) & 255u))
+    return fail(SA_ERR_WORKSPACE, "sa_block_sparse_attn_fwd_host: scratch %zu B < %zu B or not 256 B aligned",
+                scratch_bytes, need);
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const size_t tb = static_cast<size_t>(B) * H * N * D * 2, t = al256(tb);
+  const size_t lb = static_cast<size_t>(B) * H * N * 4, l = al256(lb);
+  const size_t mb = static_cast<size_t>(H) * (N / Bq) * ((N / Bk + 31) / 32) * 4, m = al256(mb);
+  char* base = static_cast<char*>(scratch);
+  char *dq = base, *dk = base + t, *dv = base + 2 * t, *dout = base + 3 * t;
+  char* dlse = base + 4 * t;
+  char* dmask = dlse + l;
+  char* dws = dmask + m;
+  cudaError_t e;
+  if ((e = cudaMemcpyAsync(dq, q_host, tb, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+      (e = cudaMemcpyAsync(dk, k_host, tb, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+      (e = cudaMemcpyAsync(dv, v_host, tb, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+      (e = cudaMemcpyAsync(dmask, mask_bits_host, mb, cudaMemcpyHostToDevice, st)) != cudaSuccess)
+    return cuda_fail(e, "host->device copy");
+  s = sa_block_sparse_attn_fwd_ex(dq, dk, dv, reinterpret_cast<const uint32_t*>(dmask), dout,
+                                  reinterpret_cast<float*>(dlse), B, H, N, n_valid, D, Bq, Bk,
+                                  scale, dws, sa_fwd_workspace_bytes(B, H, N, Bq), stream);
+  if (s != SA_OK) return s;
+  if ((e = cudaMemcpyAsync(out_host, dout, tb, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+      (e = cudaMemcpyAsync(lse_host, dlse, lb, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+    return cuda_fail(e, "device->host copy");
+  return SA_OK;
+}
+
+sa_status sa_enumerate_active_blocks(const uint32_t* mask_bits, int H, int NQB, int NKB,
+                                     int32_t* idx, int32_t* cnt, void* stream) {
+  if (!mask_bits || !idx || !cnt)
+    return fail(SA_ERR_INVALID_ARG, "sa_enumerate_active_blocks: null pointer");
+  if (H <= 0 || NQB <= 0 || NKB <= 0)
+    return fail(SA_ERR_INVALID_ARG, "sa_enumerate_active_blocks: sizes must be positive");
+  sa_status s = check_device();
+  if (s != SA_OK) return s;
+  cudaError_t e = sa::launch_enumerate(mask_bits, H, NQB, NKB, idx, cnt,
+                                       static_cast<cudaStream_t>(stream));
+  if (e != cudaSuccess) return cuda_fail(e, "sa_enumerate_active_blocks launch");
+  return SA_OK;
+}
+
+sa_status sa_set_fwd_variant(int variant) {
+  if (variant != 0 && variant != 1)
+    return fail(SA_ERR_INVALID_ARG, "sa_set_fwd_variant: variant %d not in {0,1}", variant);
+  g_variant = variant;
+  return SA_OK;
+}
+int sa_get_fwd_variant(void) { return g_variant; }
+int sa_last_launch_count(void) { return g_last_launches; }
+
+const char* sa_status_string(sa_status s) {
+  switch (s) {
+    case SA_OK: return "SA_OK";
+    case SA_ERR_INVALID_ARG: return "SA_ERR_INVALID_ARG";
+    case SA_ERR_UNSUPPORTED: return "SA_ERR_UNSUPPORTED";
+    case SA_ERR_CUDA: return "SA_ERR_CUDA";
+    case SA_ERR_WORKSPACE: return "SA_ERR_WORKSPACE";
+  }
+  return "SA_ERR_UNKNOWN";
+}
+const char* sa_last_error(void) { return g_err; }
+
+}  // extern "C"

@@ -1,0 +1,95 @@
+// common.cuh -- shared declarations of the CUDA library (product side only; the oracle never
+// includes this).
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <stdint.h>
+#include <stddef.h>
+
+#include "../../include/scalingattn.h"
+
+namespace sa {
+
+// ---- CRM forward iterator (App. E Alg. 2), one instance per walking thread ----
+// State {ptr, end, val, base} as in the paper. INIT sets base = -32 and prefetches the first
+// non-zero word; ADVANCE skips zero words (base += 32 per word); INDEX = base + CTZ(val), here
+// __ffs(val) - 1; NEXT clears the lowest set bit (val &= val - 1). The last word is ANDed with the
+// valid-bit mask so stray bits at positions >= NKB cannot index past the last key block.
+struct CrmIter {
+  const uint32_t* ptr;
+  const uint32_t* end;
+  uint32_t val;
+  uint32_t tail_mask;
+  int base;
+
+  __device__ __forceinline__ void advance() {
+    while (val == 0u && ptr != end) {
+      val = __ldg(ptr);
+      ++ptr;
+      if (ptr == end) val &= tail_mask;
+      base += 32;
+    }
+  }
+  __device__ __forceinline__ void init(const uint32_t* row_ptr, int n_words, int nkb) {
+    ptr = row_ptr;
+    end = row_ptr + n_words;
+    val = 0u;
+    base = -32;
+    tail_mask = (nkb & 31) ? ((1u << (nkb & 31)) - 1u) : 0xFFFFFFFFu;
+    advance();
+  }
+  // -1 is the end-of-row sentinel
+  __device__ __forceinline__ int index() const { return val ? base + (__ffs(val) - 1) : -1; }
+  __device__ __forceinline__ void next() {
+    val &= val - 1u;
+    if (val == 0u) advance();
+  }
+};
+
+// ---- forward-pass problem description handed to the kernels ----
+struct FwdParams {
+  const __nv_bfloat16* q;
+  const __nv_bfloat16* k;
+  const __nv_bfloat16* v;
+  const uint32_t* mask_bits;
+  __nv_bfloat16* out;
+  float* lse;
+  int B, H, N, n_valid, D, Bq, Bk;
+  int NQB, NKB, W;
+  float scale;
+  float scale_log2;   // scale * log2(e)
+  // schedule (workspace)
+  const int32_t* unit_order;  // [n_items] item ids in issue order
+  int32_t* counter;           // dynamic scheduler cursor (zeroed by the pre-pass)
+  int n_items;
+};
+
+// Workspace layout for the forward pass (all int32):
+//   [0]                  scheduler cursor
+//   [16 .. 16+BH)        per-(b,h) total cost
+//   [.. + BH)            (b,h) issue order (heaviest first)
+//   [.. + BH*items]      per-(b,h) item order (cost descending), local item index
+//   [.. + BH*items]      flattened issue order of global item ids
+struct FwdWorkspace {
+  int32_t* cursor;
+  int32_t* head_cost;
+  int32_t* head_order;
+  int32_t* local_order;
+  int32_t* unit_order;
+};
+size_t fwd_workspace_bytes(int B, int H, int NQB);
+FwdWorkspace carve_fwd_workspace(void* ws, int B, int H, int NQB);
+
+// launchers (each returns the cudaError_t of its launches; *n_launch += kernels enqueued)
+cudaError_t launch_schedule(const FwdParams& p, const FwdWorkspace& w, int rows_per_item,
+                            cudaStream_t st, int* n_launch);
+cudaError_t launch_fwd_mma_sync(const FwdParams& p, cudaStream_t st, int* n_launch);
+cudaError_t launch_fwd_tcgen05(const FwdParams& p, void* ws_extra, cudaStream_t st, int* n_launch,
+                               const char** err_text);
+cudaError_t launch_pack_mask(const float* scores, const float* density, uint32_t* mask_bits, int H,
+                             int NQB, int NKB, int force_diag, void* ws, cudaStream_t st);
+size_t pack_mask_workspace_bytes(int H, int NQB, int NKB);
+cudaError_t launch_enumerate(const uint32_t* mask_bits, int H, int NQB, int NKB, int32_t* idx,
+                             int32_t* cnt, cudaStream_t st);
+
+}  // namespace sa
