@@ -1,8 +1,510 @@
-// placeholder, replaced by the tcgen05 kernel
+// fwd_tcgen05.cu -- block-sparse attention forward for (D,Bq,Bk) = (128,128,128) on sm_100a:
+// TMA-fed shared-memory ring, tcgen05.mma with accumulators in TMEM, warp-specialised online softmax.
+//
+// What it computes: the crm kernel of the paper (Sec. 4.3.2) -- FlashAttention's
+// forward pass with the dense KV-block iterator replaced by the CRM bit-row iterator (Alg. 2,
+// PAPER.md:484-539). Masked key blocks are never loaded and never multiplied.
+//
+// How (this design is for B200, not the paper's):
+//   * persistent grid, one CTA per SM; a work item is a PAIR of adjacent query blocks (2u, 2u+1)
+//     of one (batch, head). Items are pulled from the popcount-ordered list of the schedule
+//     pre-pass with an atomic cursor, so uneven rows and heads balance out.
+//   * the two query tiles have different bit-rows; the CTA walks the UNION of the two rows, stages
+//     each K/V tile of the union ONCE (TMA, 128B swizzle, 5-slot ring of 32 KB tiles), and issues
+//     the MMAs of a tile only where that tile's own bit is set. Adjacent query blocks of a
+//     3D-local mask share most key blocks, so L2->SM traffic per active block nearly halves.
+//   * warp 0: scheduler + TMA producer; warp 1: tcgen05.mma issuer (one thread); warp 2: TMEM
+//     allocator; warps 4-7 / 8-11: softmax warpgroups of query tile 0 / 1 (one thread per row).
+//   * TMEM (512 columns): S0 [0,128) S1 [128,256) O0 [256,384) O1 [384,512), fp32. P (bf16, two
+//     per column) overwrites the first 64 columns of its S and feeds the PV MMA as the TMEM
+//     A operand, so P never touches shared memory.
+//   * MMA issue order S0(j) PV1(j-1) S1(j) PV0(j): the softmax of one tile overlaps the MMAs of
+//     the other.
+//   * online softmax in the log2 domain with the scale folded into one FFMA; the running max is
+//     only raised when it grows by more than 8 (factor 256), which keeps the O accumulator
+//     rescale (a TMEM round trip) off the common path without changing the result beyond fp32
+//     rounding: out and lse use the same (possibly stale) max consistently.
+#include <cuda.h>
+
 #include "common.cuh"
+#include "ptx.cuh"
+
 namespace sa {
-cudaError_t launch_fwd_tcgen05(const FwdParams&, void*, cudaStream_t, int*, const char** err_text) {
-  *err_text = "tcgen05 forward kernel not built yet";
-  return cudaErrorNotSupported;
+namespace {
+
+using namespace ptx;
+
+constexpr int kBlk = 128;                 // Bq = Bk
+constexpr int kD = 128;
+constexpr int kThreads = 384;
+constexpr uint32_t kTileBytes = kBlk * kD * 2;      // 32 KB
+constexpr uint32_t kHalfBytes = kTileBytes / 2;     // one [128][64] swizzle-128B box
+constexpr int kSlots = 5;                 // K/V ring
+constexpr int kSched = 2;                 // scheduler ring
+constexpr uint32_t kTmemCols = 512;
+constexpr float kRescaleThreshold = 8.0f; // log2 units
+
+// shared memory map (offsets from a 1024 B aligned base)
+constexpr uint32_t kOffQ = 0;                                   // 2 query tiles
+constexpr uint32_t kOffRing = 2 * kTileBytes;                   // kSlots tiles
+constexpr uint32_t kOffCtl = kOffRing + kSlots * kTileBytes;    // barriers etc.
+struct __align__(8) Ctl {
+  uint64_t q_full, q_empty;
+  uint64_t kv_full[kSlots], kv_empty[kSlots];
+  uint64_t s_full[2], p_full[2], o_full[2], o_free[2];
+  uint64_t sched_full[kSched], sched_empty[kSched];
+  int32_t sched_item[kSched];
+  uint32_t tmem_base;
+};
+constexpr uint32_t kSmemBytes = kOffCtl + sizeof(Ctl) + 1024;   // + alignment slack
+static_assert(kSmemBytes <= 232448, "exceeds 227 KB of dynamic shared memory");
+
+// tcgen05 shared-memory matrix descriptors (sm_100 format: start>>4 [0,14), LBO>>4 [16,30),
+// SBO>>4 [32,46), version=1 [46,48), layout type [61,64) with 2 = 128B swizzle).
+//  K-major operand (Q, K: rows x 64 bf16 per box, 8-row groups 1024 B apart)
+constexpr uint64_t kDescKMajor = (uint64_t(1) << 16) | (uint64_t(1024 >> 4) << 32) |
+                                 (uint64_t(1) << 46) | (uint64_t(2) << 61);
+//  MN-major operand (V as B of P.V: 64 head-dim columns contiguous, key rows 128 B apart,
+//  8-key groups 1024 B apart (SBO), the next 64 head-dim columns one box = 16 KB further (LBO))
+constexpr uint64_t kDescMNMajor = (uint64_t(kHalfBytes >> 4) << 16) | (uint64_t(1024 >> 4) << 32) |
+                                  (uint64_t(1) << 46) | (uint64_t(2) << 61);
+__device__ __forceinline__ uint64_t make_desc(uint64_t base, uint32_t smem_addr) {
+  return base | static_cast<uint64_t>((smem_addr & 0x3FFFFu) >> 4);
 }
+// instruction descriptor: fp32 accumulate [4,6)=1, A,B bf16 [7,10)=[10,13)=1, B major bit 16,
+// N>>3 at [17,23), M>>4 at [24,29)
+constexpr uint32_t kIdescQK = (1u << 4) | (1u << 7) | (1u << 10) | ((128u >> 3) << 17) |
+                              ((128u >> 4) << 24);
+constexpr uint32_t kIdescPV = kIdescQK | (1u << 16);
+
+struct Item {
+  int bh, h, u0;
+  bool has1;
+  int row0;            // first token row of the (b,h) slab in the [B*H*N][D] view
+};
+__device__ __forceinline__ Item decode_item(const FwdParams& p, int item, int items_per_head) {
+  Item it;
+  it.bh = item / items_per_head;
+  it.h = it.bh % p.H;
+  it.u0 = 2 * (item % items_per_head);
+  it.has1 = it.u0 + 1 < p.NQB;
+  it.row0 = it.bh * p.N;
+  return it;
+}
+
+// word w of the bit-row of query block u (0 beyond the grid), stray high bits cleared
+__device__ __forceinline__ uint32_t row_word(const FwdParams& p, int h, int u, int w, bool exists) {
+  if (!exists) return 0u;
+  uint32_t x = __ldg(p.mask_bits + (static_cast<size_t>(h) * p.NQB + u) * p.W + w);
+  if (w == p.W - 1 && (p.NKB & 31)) x &= (1u << (p.NKB & 31)) - 1u;
+  return x;
+}
+
+struct Ring {
+  int slot = 0;
+  uint32_t phase = 0;
+  __device__ __forceinline__ void advance() {
+    if (++slot == kSlots) { slot = 0; phase ^= 1u; }
+  }
+};
+
+// ------------------------------------------------------------------ warp 0: scheduler + TMA
+__device__ void producer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, const CUtensorMap* tm_q,
+                         const CUtensorMap* tm_k, const CUtensorMap* tm_v, int items_per_head) {
+  Ring ring;
+  uint32_t q_phase = 0;
+  int sched_n = 0;
+  for (;;) {
+    const int idx = atomicAdd(p.counter, 1);
+    const int item = idx < p.n_items ? __ldg(p.unit_order + idx) : -1;
+    const int ss = sched_n % kSched;
+    mbar_wait(smem_u32(&ctl->sched_empty[ss]), ((sched_n / kSched) & 1) ^ 1u, 1);
+    ctl->sched_item[ss] = item;
+    mbar_arrive(smem_u32(&ctl->sched_full[ss]));
+    ++sched_n;
+    if (item < 0) break;
+    const Item it = decode_item(p, item, items_per_head);
+
+    mbar_wait(smem_u32(&ctl->q_empty), q_phase ^ 1u, 2);
+    const uint32_t qf = smem_u32(&ctl->q_full);
+    mbar_expect_tx(qf, it.has1 ? 2 * kTileBytes : kTileBytes);
+    for (int t = 0; t < (it.has1 ? 2 : 1); ++t) {
+      const uint32_t dst = smem_base + kOffQ + t * kTileBytes;
+      const int y = it.row0 + (it.u0 + t) * kBlk;
+      tma_load_2d(dst, tm_q, 0, y, qf);
+      tma_load_2d(dst + kHalfBytes, tm_q, 64, y, qf);
+    }
+    q_phase ^= 1u;
+
+    for (int w = 0; w < p.W; ++w) {
+      uint32_t x = row_word(p, it.h, it.u0, w, true) | row_word(p, it.h, it.u0 + 1, w, it.has1);
+      while (x) {
+        const int j = w * 32 + (__ffs(x) - 1);
+        x &= x - 1u;
+        const int y = it.row0 + j * kBlk;
+#pragma unroll
+        for (int kv = 0; kv < 2; ++kv) {
+          const uint32_t full = smem_u32(&ctl->kv_full[ring.slot]);
+          mbar_wait(smem_u32(&ctl->kv_empty[ring.slot]), ring.phase ^ 1u, 3);
+          mbar_expect_tx(full, kTileBytes);
+          const uint32_t dst = smem_base + kOffRing + ring.slot * kTileBytes;
+          const CUtensorMap* tm = kv == 0 ? tm_k : tm_v;
+          tma_load_2d(dst, tm, 0, y, full);
+          tma_load_2d(dst + kHalfBytes, tm, 64, y, full);
+          ring.advance();
+        }
+      }
+    }
+  }
+  // every MMA that reads shared memory has retired before the CTA exits
+  mbar_wait(smem_u32(&ctl->q_empty), q_phase ^ 1u, 4);
+}
+
+// ------------------------------------------------------------------ warp 1: MMA issuer
+__device__ __forceinline__ void issue_qk(uint32_t tmem_s, uint32_t q_addr, uint32_t k_addr) {
+#pragma unroll
+  for (int kk = 0; kk < kD / 16; ++kk) {
+    const uint32_t off = (kk >> 2) * kHalfBytes + (kk & 3) * 32;
+    mma_ss(tmem_s, make_desc(kDescKMajor, q_addr + off), make_desc(kDescKMajor, k_addr + off),
+           kIdescQK, kk > 0);
+  }
+}
+__device__ __forceinline__ void issue_pv(uint32_t tmem_o, uint32_t tmem_p, uint32_t v_addr,
+                                         bool accumulate) {
+#pragma unroll
+  for (int kk = 0; kk < kBlk / 16; ++kk)
+    mma_ts(tmem_o, tmem_p + kk * 8, make_desc(kDescMNMajor, v_addr + kk * 16 * 128), kIdescPV,
+           accumulate || kk > 0);
+}
+
+__device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uint32_t tmem,
+                           int items_per_head) {
+  Ring ring;
+  uint32_t q_phase = 0, sp_phase[2] = {0, 0}, o_phase[2] = {0, 0};
+  int sched_n = 0;
+  const uint32_t tm_s[2] = {tmem + 0, tmem + 128}, tm_o[2] = {tmem + 256, tmem + 384};
+  for (;;) {
+    const int ss = sched_n % kSched;
+    mbar_wait(smem_u32(&ctl->sched_full[ss]), (sched_n / kSched) & 1, 10);
+    const int item = ctl->sched_item[ss];
+    mbar_arrive(smem_u32(&ctl->sched_empty[ss]));
+    ++sched_n;
+    if (item < 0) break;
+    const Item it = decode_item(p, item, items_per_head);
+
+    mbar_wait(smem_u32(&ctl->q_full), q_phase, 11);
+    q_phase ^= 1u;
+    tc_fence_after();
+    bool started[2] = {false, false};    // tile has accumulated into O in this item
+    int pend_v = -1;                     // V slot of the PV1 still to issue
+    // the p_full wait of tile t's block j, then PV_t(j)
+    auto do_pv = [&](int t, int vslot) {
+      if (!started[t]) mbar_wait(smem_u32(&ctl->o_free[t]), o_phase[t] ^ 1u, 12);
+      mbar_wait(smem_u32(&ctl->p_full[t]), sp_phase[t], 13);
+      sp_phase[t] ^= 1u;
+      tc_fence_after();
+      issue_pv(tm_o[t], tm_s[t], smem_base + kOffRing + vslot * kTileBytes, started[t]);
+      started[t] = true;
+    };
+    for (int w = 0; w < p.W; ++w) {
+      const uint32_t x0 = row_word(p, it.h, it.u0, w, true);
+      const uint32_t x1 = row_word(p, it.h, it.u0 + 1, w, it.has1);
+      uint32_t x = x0 | x1;
+      while (x) {
+        const int bit = __ffs(x) - 1;
+        x &= x - 1u;
+        const bool a = (x0 >> bit) & 1u, b = (x1 >> bit) & 1u;
+        const int kslot = ring.slot;
+        const uint32_t kphase = ring.phase;
+        ring.advance();
+        const int vslot = ring.slot;
+        const uint32_t vphase = ring.phase;
+        ring.advance();
+        const uint32_t k_addr = smem_base + kOffRing + kslot * kTileBytes;
+
+        mbar_wait(smem_u32(&ctl->kv_full[kslot]), kphase, 14);
+        tc_fence_after();
+        if (a) {
+          issue_qk(tm_s[0], smem_base + kOffQ, k_addr);
+          tc_commit(smem_u32(&ctl->s_full[0]));
+        }
+        if (pend_v >= 0) {
+          do_pv(1, pend_v);
+          tc_commit(smem_u32(&ctl->kv_empty[pend_v]));
+          pend_v = -1;
+        }
+        if (b) {
+          issue_qk(tm_s[1], smem_base + kOffQ + kTileBytes, k_addr);
+          tc_commit(smem_u32(&ctl->s_full[1]));
+        }
+        tc_commit(smem_u32(&ctl->kv_empty[kslot]));
+        mbar_wait(smem_u32(&ctl->kv_full[vslot]), vphase, 15);
+        tc_fence_after();
+        if (a) do_pv(0, vslot);
+        if (b) pend_v = vslot;
+        else tc_commit(smem_u32(&ctl->kv_empty[vslot]));
+      }
+    }
+    if (pend_v >= 0) {
+      do_pv(1, pend_v);
+      tc_commit(smem_u32(&ctl->kv_empty[pend_v]));
+    }
+    tc_commit(smem_u32(&ctl->q_empty));
+#pragma unroll
+    for (int t = 0; t < 2; ++t)
+      if (started[t]) {
+        tc_commit(smem_u32(&ctl->o_full[t]));
+        o_phase[t] ^= 1u;
+      }
+  }
+}
+
+// ------------------------------------------------------------------ warps 4-11: softmax + epilogue
+// One thread per query row: thread (quarter, lane) of warpgroup t owns TMEM lane 32*quarter+lane
+// of S_t / O_t, so row max and row sum need no shuffles.
+__device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t tmem, int t, int quarter,
+                           int lane, int items_per_head) {
+  const int row = quarter * 32 + lane;
+  const uint32_t lane_base = static_cast<uint32_t>(quarter * 32) << 16;
+  const uint32_t tm_s = tmem + lane_base + t * 128;
+  const uint32_t tm_o = tmem + lane_base + 256 + t * 128;
+  const float c = p.scale_log2;
+  uint32_t sp_phase = 0, o_phase = 0;
+  int sched_n = 0;
+  for (;;) {
+    const int ss = sched_n % kSched;
+    mbar_wait(smem_u32(&ctl->sched_full[ss]), (sched_n / kSched) & 1, 20);
+    const int item = ctl->sched_item[ss];
+    __syncwarp();
+    if (lane == 0) mbar_arrive(smem_u32(&ctl->sched_empty[ss]));
+    ++sched_n;
+    if (item < 0) break;
+    const Item it = decode_item(p, item, items_per_head);
+    const int u = it.u0 + t;
+    if (u >= p.NQB) continue;
+
+    float m_run = -INFINITY, l_run = 0.f;
+    bool started = false;
+    for (int w = 0; w < p.W; ++w) {
+      uint32_t x = row_word(p, it.h, u, w, true);
+      while (x) {
+        const int j = w * 32 + (__ffs(x) - 1);
+        x &= x - 1u;
+        mbar_wait(smem_u32(&ctl->s_full[t]), sp_phase, 21);
+        sp_phase ^= 1u;
+        tc_fence_after();
+        uint32_t sr[4][32];
+#pragma unroll
+        for (int cc = 0; cc < 4; ++cc) tmem_ld32(tm_s + cc * 32, sr[cc]);
+        tc_wait_ld();
+        // keys >= n_valid carry zero weight (only the ragged tail block can hold any)
+        const int kv = p.n_valid - j * kBlk;
+        if (kv < kBlk) {
+#pragma unroll
+          for (int cc = 0; cc < 4; ++cc)
+#pragma unroll
+            for (int i = 0; i < 32; ++i)
+              if (cc * 32 + i >= kv) sr[cc][i] = 0xFF800000u;   // -inf
+        }
+        float mx = -INFINITY;
+#pragma unroll
+        for (int cc = 0; cc < 4; ++cc)
+#pragma unroll
+          for (int i = 0; i < 32; ++i) mx = fmaxf(mx, __uint_as_float(sr[cc][i]));
+        const float m_new = mx * c;
+        const bool need = m_new > m_run + kRescaleThreshold;   // also true for the first finite max
+        if (__any_sync(0xFFFFFFFFu, need)) {
+          float alpha = 1.f;
+          if (need) {
+            alpha = ex2(m_run - m_new);      // m_run = -inf -> 0
+            m_run = m_new;
+            l_run *= alpha;
+          }
+          if (started) {                     // O_t holds earlier blocks: bring it to the new max
+#pragma unroll
+            for (int cc = 0; cc < 4; ++cc) {
+              uint32_t orr[32];
+              tmem_ld32(tm_o + cc * 32, orr);
+              tc_wait_ld();
+#pragma unroll
+              for (int i = 0; i < 32; ++i) orr[i] = __float_as_uint(__uint_as_float(orr[i]) * alpha);
+              tmem_st32(tm_o + cc * 32, orr);
+            }
+          }
+        }
+        const float m_use = (m_run == -INFINITY) ? 0.f : m_run;
+#pragma unroll
+        for (int cc = 0; cc < 4; ++cc) {
+          uint32_t pk[16];
+#pragma unroll
+          for (int i = 0; i < 16; ++i) {
+            const float p0 = ex2(fmaf(__uint_as_float(sr[cc][2 * i]), c, -m_use));
+            const float p1 = ex2(fmaf(__uint_as_float(sr[cc][2 * i + 1]), c, -m_use));
+            l_run += p0 + p1;
+            pk[i] = pack_bf16x2(p0, p1);
+          }
+          tmem_st16(tm_s + cc * 16, pk);
+        }
+        tc_wait_st();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&ctl->p_full[t]));
+        started = true;
+      }
+    }
+
+    // ---- epilogue: O / l -> bf16, lse = ln2 * (m + log2 l); empty row -> 0 / -inf
+    const size_t grow = static_cast<size_t>(it.row0) + static_cast<size_t>(u) * kBlk + row;
+    uint4* orow = reinterpret_cast<uint4*>(p.out + grow * kD);
+    if (started) {
+      mbar_wait(smem_u32(&ctl->o_full[t]), o_phase, 22);
+      o_phase ^= 1u;
+      tc_fence_after();
+      const float inv = l_run > 0.f ? 1.f / l_run : 0.f;
+#pragma unroll
+      for (int cc = 0; cc < 4; ++cc) {
+        uint32_t orr[32];
+        tmem_ld32(tm_o + cc * 32, orr);
+        tc_wait_ld();
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          uint4 v;
+          v.x = pack_bf16x2(__uint_as_float(orr[8 * i + 0]) * inv, __uint_as_float(orr[8 * i + 1]) * inv);
+          v.y = pack_bf16x2(__uint_as_float(orr[8 * i + 2]) * inv, __uint_as_float(orr[8 * i + 3]) * inv);
+          v.z = pack_bf16x2(__uint_as_float(orr[8 * i + 4]) * inv, __uint_as_float(orr[8 * i + 5]) * inv);
+          v.w = pack_bf16x2(__uint_as_float(orr[8 * i + 6]) * inv, __uint_as_float(orr[8 * i + 7]) * inv);
+          orow[cc * 4 + i] = v;
+        }
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(smem_u32(&ctl->o_free[t]));
+      p.lse[grow] = l_run > 0.f ? 0.6931471805599453f * (m_run + lg2(l_run)) : -INFINITY;
+    } else {
+      const uint4 z = make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll
+      for (int i = 0; i < 16; ++i) orow[i] = z;
+      p.lse[grow] = -INFINITY;
+    }
+  }
+}
+
+// ------------------------------------------------------------------ kernel
+__global__ void __launch_bounds__(kThreads, 1)
+fwd_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
+                   const __grid_constant__ CUtensorMap tm_v, const FwdParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t raw = smem_u32(smem_raw);
+  const uint32_t smem_base = (raw + 1023u) & ~1023u;
+  Ctl* ctl = reinterpret_cast<Ctl*>(smem_raw + (smem_base - raw) + kOffCtl);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int items_per_head = (p.NQB + 1) / 2;
+
+  if (threadIdx.x == 0) {
+    prefetch_tensormap(&tm_q);
+    prefetch_tensormap(&tm_k);
+    prefetch_tensormap(&tm_v);
+    mbar_init(smem_u32(&ctl->q_full), 1);
+    mbar_init(smem_u32(&ctl->q_empty), 1);
+    for (int s = 0; s < kSlots; ++s) {
+      mbar_init(smem_u32(&ctl->kv_full[s]), 1);
+      mbar_init(smem_u32(&ctl->kv_empty[s]), 1);
+    }
+    for (int t = 0; t < 2; ++t) {
+      mbar_init(smem_u32(&ctl->s_full[t]), 1);
+      mbar_init(smem_u32(&ctl->p_full[t]), 4);     // one arrival per softmax warp
+      mbar_init(smem_u32(&ctl->o_full[t]), 1);
+      mbar_init(smem_u32(&ctl->o_free[t]), 4);
+    }
+    for (int s = 0; s < kSched; ++s) {
+      mbar_init(smem_u32(&ctl->sched_full[s]), 1);
+      mbar_init(smem_u32(&ctl->sched_empty[s]), 9);  // MMA thread + 8 softmax warps
+    }
+    fence_mbar_init();
+  }
+  if (warp == 2) {
+    tmem_alloc(smem_u32(&ctl->tmem_base), kTmemCols);
+    tmem_relinquish();
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = ctl->tmem_base;
+
+  if (warp < 4) {
+    setmaxnreg_dec<88>();
+    if (warp == 0) {
+      if (lane == 0) producer(p, ctl, smem_base, &tm_q, &tm_k, &tm_v, items_per_head);
+    } else if (warp == 1) {
+      if (lane == 0) mma_issuer(p, ctl, smem_base, tmem, items_per_head);
+    }
+  } else {
+    setmaxnreg_inc<208>();
+    softmax_wg(p, ctl, tmem, warp >= 8 ? 1 : 0, warp & 3, lane, items_per_head);
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 2) tmem_dealloc(tmem, kTmemCols);
+}
+
+// ------------------------------------------------------------------ host side
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
+                                  const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = [] {
+    void* f = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+      f = nullptr;
+    return reinterpret_cast<EncodeTiledFn>(f);
+  }();
+  return fn;
+}
+
+// [rows][128] bf16 row-major viewed as a 2-D tensor; box = 64 columns x 128 rows, 128B swizzle
+bool make_map(CUtensorMap* m, const void* base, uint64_t rows) {
+  EncodeTiledFn fn = encode_fn();
+  if (!fn) return false;
+  const cuuint64_t gdim[2] = {static_cast<cuuint64_t>(kD), rows};
+  const cuuint64_t gstride[1] = {static_cast<cuuint64_t>(kD) * 2};
+  const cuuint32_t box[2] = {64, static_cast<cuuint32_t>(kBlk)};
+  const cuuint32_t estr[2] = {1, 1};
+  return fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), gdim, gstride, box,
+            estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+            CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+}  // namespace
+
+cudaError_t launch_fwd_tcgen05(const FwdParams& p, void*, cudaStream_t st, int* n_launch,
+                               const char** err_text) {
+  static int n_sm = 0;
+  static bool attr_set = false;
+  if (!attr_set) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(fwd_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             static_cast<int>(kSmemBytes));
+    if (e != cudaSuccess) { *err_text = "cudaFuncSetAttribute(fwd_tcgen05_kernel)"; return e; }
+    attr_set = true;
+  }
+  CUtensorMap tq, tk, tv;
+  const uint64_t rows = static_cast<uint64_t>(p.B) * p.H * p.N;
+  if (!make_map(&tq, p.q, rows) || !make_map(&tk, p.k, rows) || !make_map(&tv, p.v, rows)) {
+    *err_text = "cuTensorMapEncodeTiled failed";
+    return cudaErrorInvalidValue;
+  }
+  const int grid = p.n_items < n_sm ? p.n_items : n_sm;
+  fwd_tcgen05_kernel<<<grid, kThreads, kSmemBytes, st>>>(tq, tk, tv, p);
+  *n_launch += 1;
+  return cudaGetLastError();
+}
+
 }  // namespace sa
