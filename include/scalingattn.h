@@ -103,6 +103,28 @@ SA_API sa_status sa_block_sparse_attn_fwd_host(const void* q_host, const void* k
                                         int Bq, int Bk, float scale, void* scratch,
                                         size_t scratch_bytes, void* stream);
 
+/* One pass of the whole hot path with HOST buffers (pinned memory recommended), all on `stream`,
+ * without synchronising: copies scores [H][NQB][NKB] and density [H] to the device and packs the
+ * mask (sa_pack_mask, force_diag as there), copies q, k, v, runs the forward pass, and copies out,
+ * lse and the packed mask (mask_bits_host, uint32 [H][NQB][W], out) back. `scratch` is device
+ * memory of at least sa_hot_path_host_scratch_bytes(...) bytes, 256 B aligned. */
+SA_API size_t sa_hot_path_host_scratch_bytes(int B, int H, int N, int D, int Bq, int Bk);
+SA_API sa_status sa_hot_path_host(const float* scores_host, const float* density_host, int force_diag,
+                           const void* q_host, const void* k_host, const void* v_host,
+                           uint32_t* mask_bits_host, void* out_host, float* lse_host, int B, int H,
+                           int N, int n_valid, int D, int Bq, int Bk, float scale, void* scratch,
+                           size_t scratch_bytes, void* stream);
+
+/* Device timing of the dominant kernel. sa_profile_enable(capacity > 0) creates `capacity` CUDA
+ * event pairs; from then on each forward call records one pair on its stream around the
+ * attention kernel alone (after the schedule pre-pass), until `capacity` calls have been recorded.
+ * sa_profile_collect waits for the recorded pairs, writes their elapsed milliseconds to
+ * ms_host[0..*count_host) (host memory, at most `capacity` entries) and starts over at pair 0.
+ * sa_profile_enable(0) switches recording off and destroys the events. Process-wide; not for use
+ * from several threads at once. */
+SA_API sa_status sa_profile_enable(int capacity);
+SA_API sa_status sa_profile_collect(float* ms_host, int capacity, int* count_host);
+
 /* CRM forward iterator on the device (Alg. 2), exposed so that its walk can be
  * checked on its own: for every row (h,u) writes the active key blocks in the order the iterator
  * yields them to idx[h][u][0..cnt) (int32 [H][NQB][NKB]) and their number to cnt[h][u]
@@ -117,7 +139,8 @@ SA_API sa_status sa_enumerate_active_blocks(const uint32_t* mask_bits, int H, in
 SA_API sa_status sa_set_fwd_variant(int variant);
 SA_API int sa_get_fwd_variant(void);
 
-/* Number of kernels the last forward call on this thread enqueued (for bench accounting). */
+/* Number of kernels the last sa_pack_mask / forward / sa_hot_path_host call on this thread
+ * enqueued (for bench accounting; memsets and copies are not counted). */
 SA_API int sa_last_launch_count(void);
 
 SA_API const char* sa_status_string(sa_status s); /* static string, never freed */

@@ -59,6 +59,15 @@ def load_library() -> C.CDLL:
     lib.sa_block_sparse_attn_fwd_host.restype = ip
     lib.sa_block_sparse_attn_fwd_host.argtypes = [vp, vp, vp, vp, vp, vp, ip, ip, ip, ip, ip, ip,
                                                   ip, fp, vp, sz, vp]
+    lib.sa_hot_path_host_scratch_bytes.restype = sz
+    lib.sa_hot_path_host_scratch_bytes.argtypes = [ip] * 6
+    lib.sa_hot_path_host.restype = ip
+    lib.sa_hot_path_host.argtypes = [vp, vp, ip, vp, vp, vp, vp, vp, vp, ip, ip, ip, ip, ip, ip,
+                                     ip, fp, vp, sz, vp]
+    lib.sa_profile_enable.restype = ip
+    lib.sa_profile_enable.argtypes = [ip]
+    lib.sa_profile_collect.restype = ip
+    lib.sa_profile_collect.argtypes = [vp, ip, vp]
     lib.sa_enumerate_active_blocks.restype = ip
     lib.sa_enumerate_active_blocks.argtypes = [vp, ip, ip, ip, vp, vp, vp]
     lib.sa_set_fwd_variant.restype = ip
@@ -203,6 +212,42 @@ def sa_block_sparse_attn_fwd_host(q, k, v, mask_bits, out, lse, Bq: int, Bk: int
                                              float(scale), _ptr(scratch), scratch.numel(),
                                              _stream(stream)))
     return out, lse
+
+
+def sa_hot_path_host_scratch_bytes(B: int, H: int, N: int, D: int, Bq: int, Bk: int) -> int:
+    return load_library().sa_hot_path_host_scratch_bytes(B, H, N, D, Bq, Bk)
+
+
+def sa_hot_path_host(scores, density, q, k, v, mask_bits, out, lse, Bq: int, Bk: int,
+                     scale: float, n_valid, scratch, force_diag: bool = True, stream=None):
+    """Whole hot path with HOST (pinned) tensors: scores, density -> mask_bits (out, host);
+    q, k, v -> out, lse (host). scratch is a device uint8 tensor."""
+    lib = load_library()
+    B, H, N, D = _fwd_shapes(q, k, v, mask_bits, Bq, Bk)
+    for t in (scores, density, q, k, v, mask_bits, out, lse):
+        assert t.device.type == "cpu" and t.is_contiguous()
+    assert scores.dtype == torch.float32 and tuple(scores.shape) == (H, N // Bq, N // Bk)
+    assert density.dtype == torch.float32 and tuple(density.shape) == (H,)
+    assert out.dtype == torch.bfloat16 and out.shape == q.shape
+    assert lse.dtype == torch.float32 and tuple(lse.shape) == (B, H, N)
+    _check(lib.sa_hot_path_host(_ptr(scores), _ptr(density), int(bool(force_diag)), _ptr(q),
+                                _ptr(k), _ptr(v), _ptr(mask_bits), _ptr(out), _ptr(lse), B, H, N,
+                                int(n_valid), D, Bq, Bk, float(scale), _ptr(scratch),
+                                scratch.numel(), _stream(stream)))
+    return mask_bits, out, lse
+
+
+def sa_profile_enable(capacity: int) -> None:
+    _check(load_library().sa_profile_enable(int(capacity)))
+
+
+def sa_profile_collect(capacity: int):
+    """Elapsed milliseconds of the attention kernel of each forward call recorded since the last
+    collect (synchronises on them)."""
+    ms = (C.c_float * max(capacity, 1))()
+    n = C.c_int(0)
+    _check(load_library().sa_profile_collect(C.addressof(ms), capacity, C.addressof(n)))
+    return [float(ms[i]) for i in range(n.value)]
 
 
 def sa_enumerate_active_blocks(mask_bits, NKB: int, stream=None):

@@ -4,6 +4,7 @@
 #include <cstdio>
 #include <cstring>
 #include <mutex>
+#include <vector>
 
 #include "common.cuh"
 
@@ -70,6 +71,17 @@ sa_status validate_shape(int B, int H, int N, int n_valid, int D, int Bq, int Bk
   return SA_OK;
 }
 
+// optional device timing of the dominant kernel (sa_profile_enable / sa_profile_collect)
+std::mutex g_prof_mu;
+std::vector<cudaEvent_t> g_prof_ev;   // 2 * capacity events: start, stop per forward call
+int g_prof_n = 0;                     // forward calls recorded since the last collect
+
+void prof_free() {
+  for (cudaEvent_t e : g_prof_ev) cudaEventDestroy(e);
+  g_prof_ev.clear();
+  g_prof_n = 0;
+}
+
 // internal workspace of the short-signature call
 std::mutex g_ws_mu;
 void* g_ws = nullptr;
@@ -129,6 +141,7 @@ sa_status sa_pack_mask(const float* scores, const float* density, uint32_t* mask
   cudaError_t e = sa::launch_pack_mask(scores, density, mask_bits, H, NQB, NKB, force_diag ? 1 : 0,
                                        workspace, static_cast<cudaStream_t>(stream));
   if (e != cudaSuccess) return cuda_fail(e, "sa_pack_mask launch");
+  g_last_launches = sa::kPackMaskLaunches;
   return SA_OK;
 }
 
@@ -173,6 +186,16 @@ sa_status sa_block_sparse_attn_fwd_ex(const void* q, const void* k, const void* 
   p.n_items = B * H * ((p.NQB + rows_per_item - 1) / rows_per_item);
   cudaError_t e = sa::launch_schedule(p, w, rows_per_item, st, &g_last_launches);
   if (e != cudaSuccess) return cuda_fail(e, "schedule pre-pass launch");
+  cudaEvent_t ev_stop = nullptr;
+  {
+    std::lock_guard<std::mutex> lk(g_prof_mu);
+    if (2 * static_cast<size_t>(g_prof_n) + 1 < g_prof_ev.size()) {
+      e = cudaEventRecord(g_prof_ev[2 * g_prof_n], st);
+      if (e != cudaSuccess) return cuda_fail(e, "cudaEventRecord(profile start)");
+      ev_stop = g_prof_ev[2 * g_prof_n + 1];
+      ++g_prof_n;
+    }
+  }
   if (fast) {
     const char* txt = nullptr;
     e = sa::launch_fwd_tcgen05(p, nullptr, st, &g_last_launches, &txt);
@@ -180,6 +203,10 @@ sa_status sa_block_sparse_attn_fwd_ex(const void* q, const void* k, const void* 
   } else {
     e = sa::launch_fwd_mma_sync(p, st, &g_last_launches);
     if (e != cudaSuccess) return cuda_fail(e, "mma.sync forward launch");
+  }
+  if (ev_stop) {
+    e = cudaEventRecord(ev_stop, st);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaEventRecord(profile stop)");
   }
   return SA_OK;
 }
@@ -244,6 +271,99 @@ sa_status sa_block_sparse_attn_fwd_host(const void* q_host, const void* k_host, 
   if ((e = cudaMemcpyAsync(out_host, dout, tb, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
       (e = cudaMemcpyAsync(lse_host, dlse, lb, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
     return cuda_fail(e, "device->host copy");
+  return SA_OK;
+}
+
+size_t sa_hot_path_host_scratch_bytes(int B, int H, int N, int D, int Bq, int Bk) {
+  const size_t f = sa_fwd_host_scratch_bytes(B, H, N, D, Bq, Bk);
+  if (f == 0) return 0;
+  const int NQB = N / Bq, NKB = N / Bk;
+  return f + al256(static_cast<size_t>(H) * NQB * NKB * 4) + al256(static_cast<size_t>(H) * 4) +
+         al256(sa_pack_mask_workspace_bytes(H, NQB, NKB));
+}
+
+sa_status sa_hot_path_host(const float* scores_host, const float* density_host, int force_diag,
+                           const void* q_host, const void* k_host, const void* v_host,
+                           uint32_t* mask_bits_host, void* out_host, float* lse_host, int B, int H,
+                           int N, int n_valid, int D, int Bq, int Bk, float scale, void* scratch,
+                           size_t scratch_bytes, void* stream) {
+  if (!scores_host || !density_host || !q_host || !k_host || !v_host || !mask_bits_host ||
+      !out_host || !lse_host)
+    return fail(SA_ERR_INVALID_ARG, "sa_hot_path_host: null pointer");
+  sa_status s = validate_shape(B, H, N, n_valid, D, Bq, Bk, scale);
+  if (s != SA_OK) return s;
+  const size_t need = sa_hot_path_host_scratch_bytes(B, H, N, D, Bq, Bk);
+  if (!scratch || scratch_bytes < need || (reinterpret_cast<uintptr_t>(scratch) & 255u))
+    return fail(SA_ERR_WORKSPACE, "sa_hot_path_host: scratch %zu B < %zu B or not 256 B aligned",
+                scratch_bytes, need);
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const int NQB = N / Bq, NKB = N / Bk;
+  const size_t tb = static_cast<size_t>(B) * H * N * D * 2, t = al256(tb);
+  const size_t lb = static_cast<size_t>(B) * H * N * 4, l = al256(lb);
+  const size_t mb = static_cast<size_t>(H) * NQB * ((NKB + 31) / 32) * 4, m = al256(mb);
+  const size_t sb = static_cast<size_t>(H) * NQB * NKB * 4, db = static_cast<size_t>(H) * 4;
+  const size_t fwd_ws = sa_fwd_workspace_bytes(B, H, N, Bq);
+  const size_t pack_ws = sa_pack_mask_workspace_bytes(H, NQB, NKB);
+  char* base = static_cast<char*>(scratch);
+  char *dq = base, *dk = base + t, *dv = base + 2 * t, *dout = base + 3 * t;
+  char* dlse = base + 4 * t;
+  char* dmask = dlse + l;
+  char* dws = dmask + m;
+  char* dscores = dws + fwd_ws;            // fwd_ws is a multiple of 256
+  char* ddens = dscores + al256(sb);
+  char* dpws = ddens + al256(db);
+  cudaError_t e;
+  if ((e = cudaMemcpyAsync(dscores, scores_host, sb, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+      (e = cudaMemcpyAsync(ddens, density_host, db, cudaMemcpyHostToDevice, st)) != cudaSuccess)
+    return cuda_fail(e, "host->device copy (scores)");
+  s = sa_pack_mask(reinterpret_cast<const float*>(dscores), reinterpret_cast<const float*>(ddens),
+                   reinterpret_cast<uint32_t*>(dmask), H, NQB, NKB, force_diag, dpws, pack_ws,
+                   stream);
+  if (s != SA_OK) return s;
+  if ((e = cudaMemcpyAsync(dq, q_host, tb, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+      (e = cudaMemcpyAsync(dk, k_host, tb, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+      (e = cudaMemcpyAsync(dv, v_host, tb, cudaMemcpyHostToDevice, st)) != cudaSuccess)
+    return cuda_fail(e, "host->device copy (q, k, v)");
+  s = sa_block_sparse_attn_fwd_ex(dq, dk, dv, reinterpret_cast<const uint32_t*>(dmask), dout,
+                                  reinterpret_cast<float*>(dlse), B, H, N, n_valid, D, Bq, Bk,
+                                  scale, dws, fwd_ws, stream);
+  if (s != SA_OK) return s;
+  g_last_launches += sa::kPackMaskLaunches;
+  if ((e = cudaMemcpyAsync(out_host, dout, tb, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+      (e = cudaMemcpyAsync(lse_host, dlse, lb, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+      (e = cudaMemcpyAsync(mask_bits_host, dmask, mb, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+    return cuda_fail(e, "device->host copy");
+  return SA_OK;
+}
+
+sa_status sa_profile_enable(int capacity) {
+  std::lock_guard<std::mutex> lk(g_prof_mu);
+  prof_free();
+  if (capacity < 0) return fail(SA_ERR_INVALID_ARG, "sa_profile_enable: capacity %d < 0", capacity);
+  for (int i = 0; i < 2 * capacity; ++i) {
+    cudaEvent_t ev;
+    cudaError_t e = cudaEventCreate(&ev);
+    if (e != cudaSuccess) {
+      prof_free();
+      return cuda_fail(e, "cudaEventCreate");
+    }
+    g_prof_ev.push_back(ev);
+  }
+  return SA_OK;
+}
+
+sa_status sa_profile_collect(float* ms_host, int capacity, int* count_host) {
+  if (!ms_host || !count_host || capacity < 0)
+    return fail(SA_ERR_INVALID_ARG, "sa_profile_collect: bad arguments");
+  std::lock_guard<std::mutex> lk(g_prof_mu);
+  const int n = g_prof_n < capacity ? g_prof_n : capacity;
+  for (int i = 0; i < n; ++i) {
+    cudaError_t e = cudaEventSynchronize(g_prof_ev[2 * i + 1]);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms_host[i], g_prof_ev[2 * i], g_prof_ev[2 * i + 1]);
+    if (e != cudaSuccess) return cuda_fail(e, "sa_profile_collect");
+  }
+  *count_host = n;
+  g_prof_n = 0;
   return SA_OK;
 }
 
