@@ -43,6 +43,22 @@ constexpr int kSlots = 5;                 // K/V ring
 constexpr int kSched = 2;                 // scheduler ring
 constexpr uint32_t kTmemCols = 512;
 constexpr float kRescaleThreshold = 8.0f; // log2 units
+// Tunables of the softmax (defaults chosen by measurement on B200, profiles/):
+//  SA_POLY_PAIRS: of every 4 consecutive column pairs, how many take exp2 on the FMA pipe
+//  (Cody-Waite split + degree-3 polynomial) instead of MUFU.EX2 -- the MUFU pipe (16/clk/SM)
+//  would otherwise need as many cycles per tile as the two MMAs.
+//  SA_PCHUNKS: in how many pieces P is handed to the PV MMA (the MMA of the first keys starts
+//  while the exponentials of the later ones are still being computed).
+#ifndef SA_POLY_PAIRS
+#define SA_POLY_PAIRS 0
+#endif
+#ifndef SA_PCHUNKS
+#define SA_PCHUNKS 4
+#endif
+constexpr int kPolyPairs = SA_POLY_PAIRS;
+constexpr int kPChunks = SA_PCHUNKS;
+static_assert(kPolyPairs >= 0 && kPolyPairs <= 4, "SA_POLY_PAIRS in 0..4");
+static_assert(kPChunks == 1 || kPChunks == 2 || kPChunks == 4, "SA_PCHUNKS in {1,2,4}");
 
 // shared memory map (offsets from a 1024 B aligned base)
 constexpr uint32_t kOffQ = 0;                                   // 2 query tiles
@@ -51,7 +67,7 @@ constexpr uint32_t kOffCtl = kOffRing + kSlots * kTileBytes;    // barriers etc.
 struct __align__(8) Ctl {
   uint64_t q_full, q_empty;
   uint64_t kv_full[kSlots], kv_empty[kSlots];
-  uint64_t s_full[2], p_full[2], o_full[2], o_free[2];
+  uint64_t s_full[2], p_full[2][4], o_full[2], o_free[2];
   uint64_t sched_full[kSched], sched_empty[kSched];
   int32_t sched_item[kSched];
   uint32_t tmem_base;
@@ -109,30 +125,37 @@ struct Ring {
 };
 
 // ------------------------------------------------------------------ warp 0: scheduler + TMA
+// Runs on every lane of warp 0 (converged); elect.sync inside the _e wrappers picks the issuer.
 __device__ void producer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, const CUtensorMap* tm_q,
-                         const CUtensorMap* tm_k, const CUtensorMap* tm_v, int items_per_head) {
+                         const CUtensorMap* tm_k, const CUtensorMap* tm_v, int items_per_head,
+                         int lane) {
   Ring ring;
   uint32_t q_phase = 0;
   int sched_n = 0;
   for (;;) {
-    const int idx = atomicAdd(p.counter, 1);
+    int idx = 0;
+    if (lane == 0) idx = atomicAdd(p.counter, 1);
+    idx = __shfl_sync(0xFFFFFFFFu, idx, 0);
     const int item = idx < p.n_items ? __ldg(p.unit_order + idx) : -1;
     const int ss = sched_n % kSched;
     mbar_wait(smem_u32(&ctl->sched_empty[ss]), ((sched_n / kSched) & 1) ^ 1u, 1);
-    ctl->sched_item[ss] = item;
-    mbar_arrive(smem_u32(&ctl->sched_full[ss]));
+    if (lane == 0) {
+      ctl->sched_item[ss] = item;
+      mbar_arrive(smem_u32(&ctl->sched_full[ss]));
+    }
+    __syncwarp();
     ++sched_n;
     if (item < 0) break;
     const Item it = decode_item(p, item, items_per_head);
 
     mbar_wait(smem_u32(&ctl->q_empty), q_phase ^ 1u, 2);
     const uint32_t qf = smem_u32(&ctl->q_full);
-    mbar_expect_tx(qf, it.has1 ? 2 * kTileBytes : kTileBytes);
+    mbar_expect_tx_e(qf, it.has1 ? 2 * kTileBytes : kTileBytes);
     for (int t = 0; t < (it.has1 ? 2 : 1); ++t) {
       const uint32_t dst = smem_base + kOffQ + t * kTileBytes;
       const int y = it.row0 + (it.u0 + t) * kBlk;
-      tma_load_2d(dst, tm_q, 0, y, qf);
-      tma_load_2d(dst + kHalfBytes, tm_q, 64, y, qf);
+      tma_load_2d_e(dst, tm_q, 0, y, qf);
+      tma_load_2d_e(dst + kHalfBytes, tm_q, 64, y, qf);
     }
     q_phase ^= 1u;
 
@@ -146,11 +169,11 @@ __device__ void producer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, const
         for (int kv = 0; kv < 2; ++kv) {
           const uint32_t full = smem_u32(&ctl->kv_full[ring.slot]);
           mbar_wait(smem_u32(&ctl->kv_empty[ring.slot]), ring.phase ^ 1u, 3);
-          mbar_expect_tx(full, kTileBytes);
+          mbar_expect_tx_e(full, kTileBytes);
           const uint32_t dst = smem_base + kOffRing + ring.slot * kTileBytes;
           const CUtensorMap* tm = kv == 0 ? tm_k : tm_v;
-          tma_load_2d(dst, tm, 0, y, full);
-          tma_load_2d(dst + kHalfBytes, tm, 64, y, full);
+          tma_load_2d_e(dst, tm, 0, y, full);
+          tma_load_2d_e(dst + kHalfBytes, tm, 64, y, full);
           ring.advance();
         }
       }
@@ -165,20 +188,29 @@ __device__ __forceinline__ void issue_qk(uint32_t tmem_s, uint32_t q_addr, uint3
 #pragma unroll
   for (int kk = 0; kk < kD / 16; ++kk) {
     const uint32_t off = (kk >> 2) * kHalfBytes + (kk & 3) * 32;
-    mma_ss(tmem_s, make_desc(kDescKMajor, q_addr + off), make_desc(kDescKMajor, k_addr + off),
-           kIdescQK, kk > 0);
+    mma_ss_e(tmem_s, make_desc(kDescKMajor, q_addr + off), make_desc(kDescKMajor, k_addr + off),
+             kIdescQK, kk > 0);
   }
 }
+// P arrives in kPChunks pieces (p_full[c], c ascending); the MMAs of a piece are issued as soon as
+// that piece is in TMEM.
 __device__ __forceinline__ void issue_pv(uint32_t tmem_o, uint32_t tmem_p, uint32_t v_addr,
-                                         bool accumulate) {
+                                         bool accumulate, const uint64_t* p_full, uint32_t phase) {
+  constexpr int kPer = (kBlk / 16) / kPChunks;
 #pragma unroll
-  for (int kk = 0; kk < kBlk / 16; ++kk)
-    mma_ts(tmem_o, tmem_p + kk * 8, make_desc(kDescMNMajor, v_addr + kk * 16 * 128), kIdescPV,
-           accumulate || kk > 0);
+  for (int kk = 0; kk < kBlk / 16; ++kk) {
+    if (kk % kPer == 0) {
+      mbar_wait(smem_u32(&p_full[kk / kPer]), phase, 13);
+      tc_fence_after();
+    }
+    mma_ts_e(tmem_o, tmem_p + kk * 8, make_desc(kDescMNMajor, v_addr + kk * 16 * 128), kIdescPV,
+             accumulate || kk > 0);
+  }
 }
 
+// Runs on every lane of warp 1 (converged); elect.sync inside the _e wrappers picks the issuer.
 __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uint32_t tmem,
-                           int items_per_head) {
+                           int items_per_head, int lane) {
   Ring ring;
   uint32_t q_phase = 0, sp_phase[2] = {0, 0}, o_phase[2] = {0, 0};
   int sched_n = 0;
@@ -187,7 +219,8 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     const int ss = sched_n % kSched;
     mbar_wait(smem_u32(&ctl->sched_full[ss]), (sched_n / kSched) & 1, 10);
     const int item = ctl->sched_item[ss];
-    mbar_arrive(smem_u32(&ctl->sched_empty[ss]));
+    __syncwarp();
+    if (lane == 0) mbar_arrive(smem_u32(&ctl->sched_empty[ss]));
     ++sched_n;
     if (item < 0) break;
     const Item it = decode_item(p, item, items_per_head);
@@ -200,10 +233,9 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     // the p_full wait of tile t's block j, then PV_t(j)
     auto do_pv = [&](int t, int vslot) {
       if (!started[t]) mbar_wait(smem_u32(&ctl->o_free[t]), o_phase[t] ^ 1u, 12);
-      mbar_wait(smem_u32(&ctl->p_full[t]), sp_phase[t], 13);
+      issue_pv(tm_o[t], tm_s[t], smem_base + kOffRing + vslot * kTileBytes, started[t],
+               ctl->p_full[t], sp_phase[t]);
       sp_phase[t] ^= 1u;
-      tc_fence_after();
-      issue_pv(tm_o[t], tm_s[t], smem_base + kOffRing + vslot * kTileBytes, started[t]);
       started[t] = true;
     };
     for (int w = 0; w < p.W; ++w) {
@@ -226,37 +258,100 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
         tc_fence_after();
         if (a) {
           issue_qk(tm_s[0], smem_base + kOffQ, k_addr);
-          tc_commit(smem_u32(&ctl->s_full[0]));
+          tc_commit_e(smem_u32(&ctl->s_full[0]));
         }
         if (pend_v >= 0) {
           do_pv(1, pend_v);
-          tc_commit(smem_u32(&ctl->kv_empty[pend_v]));
+          tc_commit_e(smem_u32(&ctl->kv_empty[pend_v]));
           pend_v = -1;
         }
         if (b) {
           issue_qk(tm_s[1], smem_base + kOffQ + kTileBytes, k_addr);
-          tc_commit(smem_u32(&ctl->s_full[1]));
+          tc_commit_e(smem_u32(&ctl->s_full[1]));
         }
-        tc_commit(smem_u32(&ctl->kv_empty[kslot]));
+        tc_commit_e(smem_u32(&ctl->kv_empty[kslot]));
         mbar_wait(smem_u32(&ctl->kv_full[vslot]), vphase, 15);
         tc_fence_after();
         if (a) do_pv(0, vslot);
         if (b) pend_v = vslot;
-        else tc_commit(smem_u32(&ctl->kv_empty[vslot]));
+        else tc_commit_e(smem_u32(&ctl->kv_empty[vslot]));
       }
     }
     if (pend_v >= 0) {
       do_pv(1, pend_v);
-      tc_commit(smem_u32(&ctl->kv_empty[pend_v]));
+      tc_commit_e(smem_u32(&ctl->kv_empty[pend_v]));
     }
-    tc_commit(smem_u32(&ctl->q_empty));
+    tc_commit_e(smem_u32(&ctl->q_empty));
 #pragma unroll
     for (int t = 0; t < 2; ++t)
       if (started[t]) {
-        tc_commit(smem_u32(&ctl->o_full[t]));
+        tc_commit_e(smem_u32(&ctl->o_full[t]));
         o_phase[t] ^= 1u;
       }
   }
+}
+
+// 2^x for two lanes on the FMA pipe (no MUFU): x = n + f with n = floor(x) (round-down add of
+// 1.5*2^23 leaves n in the low mantissa bits), 2^f by a degree-3 polynomial with p(0) = 1 (max
+// relative error 8.6e-5 on [0,1), mean +7e-6 -- below the bf16 rounding of P), and n added to the
+// exponent field by one shift-add. x is clamped at -127 so the exponent cannot wrap.
+__device__ __forceinline__ void exp2_fma_pipe(uint64_t x, float& e0, float& e1) {
+  float x0, x1;
+  up2(x, x0, x1);
+  const uint64_t xc = pk2(fmaxf(x0, -127.f), fmaxf(x1, -127.f));
+  const uint64_t magic = pk2(12582912.f, 12582912.f);
+  const uint64_t r = add2_rm(xc, magic);
+  const uint64_t f = sub2(xc, sub2(r, magic));
+  uint64_t q = fma2(f, pk2(0.07706704f, 0.07706704f), pk2(0.22764499f, 0.22764499f));
+  q = fma2(q, f, pk2(0.69511676f, 0.69511676f));
+  q = fma2(q, f, pk2(1.f, 1.f));
+  float q0, q1, r0, r1;
+  up2(q, q0, q1);
+  up2(r, r0, r1);
+  e0 = __int_as_float(__float_as_int(q0) + (__float_as_int(r0) << 23));
+  e1 = __int_as_float(__float_as_int(q1) + (__float_as_int(r1) << 23));
+}
+
+// P = 2^(c*s - m) of one query row (128 columns in sr), written to TMEM as bf16 in kPChunks pieces
+// (p_full[piece] arrives after each); returns the row sum. Packed FFMA2 for the argument; of every
+// 4 column pairs NPOLY take the FMA-pipe exp2 and the rest MUFU.EX2 (the ragged tile uses
+// NPOLY = 0: MUFU turns its -inf columns into an exact 0). Row sum in 4 packed accumulators.
+template <int NPOLY>
+__device__ __forceinline__ float exp_tile(const uint32_t (&sr)[4][32], float c, float m_use,
+                                          uint32_t tm_p, uint64_t* p_full, int lane) {
+  const uint64_t c2 = pk2(c, c), nm2 = pk2(-m_use, -m_use);
+  uint64_t lacc[4] = {0ull, 0ull, 0ull, 0ull};
+#pragma unroll
+  for (int cc = 0; cc < 4; ++cc) {
+    uint32_t pk[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+      const uint64_t x = fma2(pk2(__uint_as_float(sr[cc][2 * i]), __uint_as_float(sr[cc][2 * i + 1])),
+                              c2, nm2);
+      float p0, p1;
+      if ((i & 3) < NPOLY) {
+        exp2_fma_pipe(x, p0, p1);
+      } else {
+        float x0, x1;
+        up2(x, x0, x1);
+        p0 = ex2(x0);
+        p1 = ex2(x1);
+      }
+      lacc[i & 3] = add2(lacc[i & 3], pk2(p0, p1));
+      pk[i] = pack_bf16x2(p0, p1);
+    }
+    tmem_st16(tm_p + cc * 16, pk);
+    if ((cc + 1) % (4 / kPChunks) == 0) {
+      tc_wait_st();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(smem_u32(&p_full[cc / (4 / kPChunks)]));
+    }
+  }
+  float a0, a1, b0, b1;
+  up2(add2(lacc[0], lacc[1]), a0, a1);
+  up2(add2(lacc[2], lacc[3]), b0, b1);
+  return (a0 + a1) + (b0 + b1);
 }
 
 // ------------------------------------------------------------------ warps 4-11: softmax + epilogue
@@ -271,6 +366,12 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t tmem, int t, i
   const float c = p.scale_log2;
   uint32_t sp_phase = 0, o_phase = 0;
   int sched_n = 0;
+#ifdef SA_TRACE
+  long long tr_acc[5] = {0, 0, 0, 0, 0}, tr_last = clock64(), tr_n = 0;
+#define SA_TR(i) { const long long now_ = clock64(); tr_acc[i] += now_ - tr_last; tr_last = now_; if (i == 4) ++tr_n; }
+#else
+#define SA_TR(i)
+#endif
   for (;;) {
     const int ss = sched_n % kSched;
     mbar_wait(smem_u32(&ctl->sched_full[ss]), (sched_n / kSched) & 1, 20);
@@ -290,28 +391,36 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t tmem, int t, i
       while (x) {
         const int j = w * 32 + (__ffs(x) - 1);
         x &= x - 1u;
+        SA_TR(0);
         mbar_wait(smem_u32(&ctl->s_full[t]), sp_phase, 21);
         sp_phase ^= 1u;
         tc_fence_after();
+        SA_TR(1);
         uint32_t sr[4][32];
 #pragma unroll
         for (int cc = 0; cc < 4; ++cc) tmem_ld32(tm_s + cc * 32, sr[cc]);
         tc_wait_ld();
+        SA_TR(2);
         // keys >= n_valid carry zero weight (only the ragged tail block can hold any)
         const int kv = p.n_valid - j * kBlk;
-        if (kv < kBlk) {
+        const bool ragged = kv < kBlk;
+        if (ragged) {
 #pragma unroll
           for (int cc = 0; cc < 4; ++cc)
 #pragma unroll
             for (int i = 0; i < 32; ++i)
               if (cc * 32 + i >= kv) sr[cc][i] = 0xFF800000u;   // -inf
         }
-        float mx = -INFINITY;
+        // row max: four independent chains of 3-input max
+        float mxa[4];
 #pragma unroll
-        for (int cc = 0; cc < 4; ++cc)
+        for (int cc = 0; cc < 4; ++cc) {
+          mxa[cc] = fmaxf(__uint_as_float(sr[cc][0]), __uint_as_float(sr[cc][1]));
 #pragma unroll
-          for (int i = 0; i < 32; ++i) mx = fmaxf(mx, __uint_as_float(sr[cc][i]));
-        const float m_new = mx * c;
+          for (int i = 2; i < 32; i += 2)
+            mxa[cc] = max3(mxa[cc], __uint_as_float(sr[cc][i]), __uint_as_float(sr[cc][i + 1]));
+        }
+        const float m_new = max3(fmaxf(mxa[0], mxa[1]), mxa[2], mxa[3]) * c;
         const bool need = m_new > m_run + kRescaleThreshold;   // also true for the first finite max
         if (__any_sync(0xFFFFFFFFu, need)) {
           float alpha = 1.f;
@@ -333,22 +442,10 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t tmem, int t, i
           }
         }
         const float m_use = (m_run == -INFINITY) ? 0.f : m_run;
-#pragma unroll
-        for (int cc = 0; cc < 4; ++cc) {
-          uint32_t pk[16];
-#pragma unroll
-          for (int i = 0; i < 16; ++i) {
-            const float p0 = ex2(fmaf(__uint_as_float(sr[cc][2 * i]), c, -m_use));
-            const float p1 = ex2(fmaf(__uint_as_float(sr[cc][2 * i + 1]), c, -m_use));
-            l_run += p0 + p1;
-            pk[i] = pack_bf16x2(p0, p1);
-          }
-          tmem_st16(tm_s + cc * 16, pk);
-        }
-        tc_wait_st();
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(smem_u32(&ctl->p_full[t]));
+        SA_TR(3);
+        if (ragged) l_run += exp_tile<0>(sr, c, m_use, tm_s, ctl->p_full[t], lane);
+        else l_run += exp_tile<kPolyPairs>(sr, c, m_use, tm_s, ctl->p_full[t], lane);
+        SA_TR(4);
         started = true;
       }
     }
@@ -387,6 +484,11 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t tmem, int t, i
       p.lse[grow] = -INFINITY;
     }
   }
+#ifdef SA_TRACE
+  if (lane == 0 && blockIdx.x < 2 && quarter == 0)
+    printf("trace cta %d wg %d blocks %lld: other+epi %lld | wait_s %lld | ld %lld | max+resc %lld | exp+st %lld (clk per block)\n",
+           blockIdx.x, t, tr_n, tr_acc[0] / tr_n, tr_acc[1] / tr_n, tr_acc[2] / tr_n, tr_acc[3] / tr_n, tr_acc[4] / tr_n);
+#endif
 }
 
 // ------------------------------------------------------------------ kernel
@@ -412,7 +514,8 @@ fwd_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
     }
     for (int t = 0; t < 2; ++t) {
       mbar_init(smem_u32(&ctl->s_full[t]), 1);
-      mbar_init(smem_u32(&ctl->p_full[t]), 4);     // one arrival per softmax warp
+      for (int c = 0; c < 4; ++c)
+        mbar_init(smem_u32(&ctl->p_full[t][c]), 4);   // one arrival per softmax warp
       mbar_init(smem_u32(&ctl->o_full[t]), 1);
       mbar_init(smem_u32(&ctl->o_free[t]), 4);
     }
@@ -434,9 +537,9 @@ fwd_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
   if (warp < 4) {
     setmaxnreg_dec<88>();
     if (warp == 0) {
-      if (lane == 0) producer(p, ctl, smem_base, &tm_q, &tm_k, &tm_v, items_per_head);
+      producer(p, ctl, smem_base, &tm_q, &tm_k, &tm_v, items_per_head, lane);
     } else if (warp == 1) {
-      if (lane == 0) mma_issuer(p, ctl, smem_base, tmem, items_per_head);
+      mma_issuer(p, ctl, smem_base, tmem, items_per_head, lane);
     }
   } else {
     setmaxnreg_inc<208>();
