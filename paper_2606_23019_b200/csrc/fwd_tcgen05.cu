@@ -53,7 +53,7 @@ constexpr float kRescaleThreshold = 8.0f; // log2 units
 #define SA_POLY_PAIRS 0
 #endif
 #ifndef SA_PCHUNKS
-#define SA_PCHUNKS 4
+#define SA_PCHUNKS 2
 #endif
 constexpr int kPolyPairs = SA_POLY_PAIRS;
 constexpr int kPChunks = SA_PCHUNKS;
@@ -67,7 +67,8 @@ constexpr uint32_t kOffCtl = kOffRing + kSlots * kTileBytes;    // barriers etc.
 struct __align__(8) Ctl {
   uint64_t q_full, q_empty;
   uint64_t kv_full[kSlots], kv_empty[kSlots];
-  uint64_t s_full[2], p_full[2][4], o_full[2], o_free[2];
+  uint64_t s_full[2][2], p_full[2][2][4], pv_done[2][2];   // [tile][tile-local unit & 1]
+  uint64_t o_full[2], o_free[2];
   uint64_t sched_full[kSched], sched_empty[kSched];
   int32_t sched_item[kSched];
   uint32_t tmem_base;
@@ -208,13 +209,52 @@ __device__ __forceinline__ void issue_pv(uint32_t tmem_o, uint32_t tmem_p, uint3
   }
 }
 
+// One (query tile, key block) unit whose S has been issued and whose PV is still to come.
+struct Pend {
+  uint32_t t, buf;             // tile, S/P buffer in TMEM
+  uint32_t sel, par;           // this unit's barriers: [t][sel], phase parity par
+  uint32_t vslot, vphase;      // ring slot holding V and the parity of its kv_full
+  uint32_t acc;                // accumulate into O_t (0 for the tile's first unit of the item)
+  uint32_t ofree_par;          // first unit only: parity of o_free[t] to wait for
+  uint32_t last_of_tile;       // last unit of this tile in its item: commit o_full[t] after the PV
+  uint32_t rel_v;              // last user of the V slot: release it after the PV
+};
+
 // Runs on every lane of warp 1 (converged); elect.sync inside the _e wrappers picks the issuer.
+//
+// Units (tile t, key block j) are numbered 0,1,2,... in walk order (ascending j over the union of
+// the two bit-rows, tile 0 before tile 1), across items. Unit w computes S into buffer w & 1 -- the
+// buffers alternate per UNIT, not per tile, so a run of key blocks that only one of the two query
+// tiles has still ping-pongs between the two S buffers. Issue order: PV(w-2), S(w): the softmax of
+// unit w-1 overlaps both. P(w-2) aliases S buffer (w & 1), so S(w) must follow PV(w-2) in the
+// (in-order) tensor pipe, which this order guarantees.
 __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uint32_t tmem,
                            int items_per_head, int lane) {
   Ring ring;
-  uint32_t q_phase = 0, sp_phase[2] = {0, 0}, o_phase[2] = {0, 0};
+  uint32_t q_phase = 0, n_started[2] = {0, 0};
+  uint32_t wg = 0;                       // global unit counter
+  uint32_t nt[2] = {0, 0};               // units issued so far per tile (barrier selection)
   int sched_n = 0;
-  const uint32_t tm_s[2] = {tmem + 0, tmem + 128}, tm_o[2] = {tmem + 256, tmem + 384};
+  Pend pd0{}, pd1{};                     // FIFO: pd0 older
+  int npend = 0;
+
+  auto issue_pend = [&](const Pend& u) {
+    if (!u.acc) mbar_wait(smem_u32(&ctl->o_free[u.t]), u.ofree_par, 12);
+    mbar_wait(smem_u32(&ctl->kv_full[u.vslot]), u.vphase, 15);
+    tc_fence_after();
+    issue_pv(tmem + 256 + u.t * 128, tmem + u.buf * 128,
+             smem_base + kOffRing + u.vslot * kTileBytes, u.acc != 0, ctl->p_full[u.t][u.sel],
+             u.par);
+    tc_commit_e(smem_u32(&ctl->pv_done[u.t][u.sel]));
+    if (u.rel_v) tc_commit_e(smem_u32(&ctl->kv_empty[u.vslot]));
+    if (u.last_of_tile) tc_commit_e(smem_u32(&ctl->o_full[u.t]));
+  };
+  auto pop = [&]() {
+    issue_pend(pd0);
+    pd0 = pd1;
+    --npend;
+  };
+
   for (;;) {
     const int ss = sched_n % kSched;
     mbar_wait(smem_u32(&ctl->sched_full[ss]), (sched_n / kSched) & 1, 10);
@@ -225,19 +265,16 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     if (item < 0) break;
     const Item it = decode_item(p, item, items_per_head);
 
+    uint32_t rem[2] = {0, 0};            // units each tile still has in this item
+    for (int w = 0; w < p.W; ++w) {
+      rem[0] += __popc(row_word(p, it.h, it.u0, w, true));
+      rem[1] += __popc(row_word(p, it.h, it.u0 + 1, w, it.has1));
+    }
+    bool first[2] = {true, true};
+
     mbar_wait(smem_u32(&ctl->q_full), q_phase, 11);
     q_phase ^= 1u;
     tc_fence_after();
-    bool started[2] = {false, false};    // tile has accumulated into O in this item
-    int pend_v = -1;                     // V slot of the PV1 still to issue
-    // the p_full wait of tile t's block j, then PV_t(j)
-    auto do_pv = [&](int t, int vslot) {
-      if (!started[t]) mbar_wait(smem_u32(&ctl->o_free[t]), o_phase[t] ^ 1u, 12);
-      issue_pv(tm_o[t], tm_s[t], smem_base + kOffRing + vslot * kTileBytes, started[t],
-               ctl->p_full[t], sp_phase[t]);
-      sp_phase[t] ^= 1u;
-      started[t] = true;
-    };
     for (int w = 0; w < p.W; ++w) {
       const uint32_t x0 = row_word(p, it.h, it.u0, w, true);
       const uint32_t x1 = row_word(p, it.h, it.u0 + 1, w, it.has1);
@@ -245,50 +282,47 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
       while (x) {
         const int bit = __ffs(x) - 1;
         x &= x - 1u;
-        const bool a = (x0 >> bit) & 1u, b = (x1 >> bit) & 1u;
+        const bool has[2] = {((x0 >> bit) & 1u) != 0, ((x1 >> bit) & 1u) != 0};
         const int kslot = ring.slot;
         const uint32_t kphase = ring.phase;
         ring.advance();
-        const int vslot = ring.slot;
+        const uint32_t vslot = ring.slot;
         const uint32_t vphase = ring.phase;
         ring.advance();
         const uint32_t k_addr = smem_base + kOffRing + kslot * kTileBytes;
-
+        if (npend == 2) pop();             // the oldest PV does not need this block's K: issue it first
         mbar_wait(smem_u32(&ctl->kv_full[kslot]), kphase, 14);
         tc_fence_after();
-        if (a) {
-          issue_qk(tm_s[0], smem_base + kOffQ, k_addr);
-          tc_commit_e(smem_u32(&ctl->s_full[0]));
-        }
-        if (pend_v >= 0) {
-          do_pv(1, pend_v);
-          tc_commit_e(smem_u32(&ctl->kv_empty[pend_v]));
-          pend_v = -1;
-        }
-        if (b) {
-          issue_qk(tm_s[1], smem_base + kOffQ + kTileBytes, k_addr);
-          tc_commit_e(smem_u32(&ctl->s_full[1]));
+#pragma unroll
+        for (int t = 0; t < 2; ++t) {
+          if (!has[t]) continue;
+          if (npend == 2) pop();
+          Pend u;
+          u.t = t;
+          u.buf = wg & 1u;
+          u.sel = nt[t] & 1u;
+          u.par = (nt[t] >> 1) & 1u;
+          ++nt[t];
+          u.vslot = vslot;
+          u.vphase = vphase;
+          u.acc = first[t] ? 0u : 1u;
+          u.ofree_par = (n_started[t] & 1u) ^ 1u;
+          u.last_of_tile = (--rem[t] == 0u) ? 1u : 0u;
+          u.rel_v = (t == 1 || !has[1]) ? 1u : 0u;
+          if (first[t]) ++n_started[t];
+          first[t] = false;
+          issue_qk(tmem + u.buf * 128, smem_base + kOffQ + t * kTileBytes, k_addr);
+          tc_commit_e(smem_u32(&ctl->s_full[t][u.sel]));
+          if (npend == 0) pd0 = u; else pd1 = u;
+          ++npend;
+          ++wg;
         }
         tc_commit_e(smem_u32(&ctl->kv_empty[kslot]));
-        mbar_wait(smem_u32(&ctl->kv_full[vslot]), vphase, 15);
-        tc_fence_after();
-        if (a) do_pv(0, vslot);
-        if (b) pend_v = vslot;
-        else tc_commit_e(smem_u32(&ctl->kv_empty[vslot]));
       }
     }
-    if (pend_v >= 0) {
-      do_pv(1, pend_v);
-      tc_commit_e(smem_u32(&ctl->kv_empty[pend_v]));
-    }
-    tc_commit_e(smem_u32(&ctl->q_empty));
-#pragma unroll
-    for (int t = 0; t < 2; ++t)
-      if (started[t]) {
-        tc_commit_e(smem_u32(&ctl->o_full[t]));
-        o_phase[t] ^= 1u;
-      }
+    tc_commit_e(smem_u32(&ctl->q_empty));   // every S of this item has been issued
   }
+  while (npend > 0) pop();
 }
 
 // 2^x for two lanes on the FMA pipe (no MUFU): x = n + f with n = floor(x) (round-down add of
@@ -340,14 +374,21 @@ __device__ __forceinline__ float exp_tile(const uint32_t (&sr)[4][32], float c, 
       lacc[i & 3] = add2(lacc[i & 3], pk2(p0, p1));
       pk[i] = pack_bf16x2(p0, p1);
     }
-    tmem_st16(tm_p + cc * 16, pk);
-    if ((cc + 1) % (4 / kPChunks) == 0) {
+    // The arrival for a piece is deferred until the next piece's exponentials are in registers:
+    // by then its tcgen05.st has long completed and wait::st does not stall.
+    constexpr int kPer = 4 / kPChunks;
+    if (cc % kPer == 0 && cc > 0) {
       tc_wait_st();
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(smem_u32(&p_full[cc / (4 / kPChunks)]));
+      if (lane == 0) mbar_arrive(smem_u32(&p_full[cc / kPer - 1]));
     }
+    tmem_st16(tm_p + cc * 16, pk);
   }
+  tc_wait_st();
+  tc_fence_before();
+  __syncwarp();
+  if (lane == 0) mbar_arrive(smem_u32(&p_full[kPChunks - 1]));
   float a0, a1, b0, b1;
   up2(add2(lacc[0], lacc[1]), a0, a1);
   up2(add2(lacc[2], lacc[3]), b0, b1);
@@ -361,14 +402,16 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t tmem, int t, i
                            int lane, int items_per_head) {
   const int row = quarter * 32 + lane;
   const uint32_t lane_base = static_cast<uint32_t>(quarter * 32) << 16;
-  const uint32_t tm_s = tmem + lane_base + t * 128;
   const uint32_t tm_o = tmem + lane_base + 256 + t * 128;
   const float c = p.scale_log2;
-  uint32_t sp_phase = 0, o_phase = 0;
+  uint32_t o_phase = 0;
+  uint32_t wg = 0;                       // global unit counter, in step with the MMA issuer
+  uint32_t nmine = 0;                    // this tile's units so far (barrier selection: every phase
+                                         // of s_full[t][.] is consumed in order, none is skipped)
   int sched_n = 0;
 #ifdef SA_TRACE
-  long long tr_acc[5] = {0, 0, 0, 0, 0}, tr_last = clock64(), tr_n = 0;
-#define SA_TR(i) { const long long now_ = clock64(); tr_acc[i] += now_ - tr_last; tr_last = now_; if (i == 4) ++tr_n; }
+  uint32_t tr_acc[5] = {0, 0, 0, 0, 0}, tr_last = clock(), tr_n = 0;
+#define SA_TR(i) { const uint32_t now_ = clock(); tr_acc[i] += now_ - tr_last; tr_last = now_; if (i == 4) ++tr_n; }
 #else
 #define SA_TR(i)
 #endif
@@ -382,18 +425,28 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t tmem, int t, i
     if (item < 0) break;
     const Item it = decode_item(p, item, items_per_head);
     const int u = it.u0 + t;
-    if (u >= p.NQB) continue;
+    const bool exists = u < p.NQB;
 
     float m_run = -INFINITY, l_run = 0.f;
     bool started = false;
+    uint32_t prev_unit = 0xFFFFFFFEu;    // this tile's previous unit in the item
+    // walk the union of the two bit-rows (the unit numbering needs both), handle this tile's units
     for (int w = 0; w < p.W; ++w) {
-      uint32_t x = row_word(p, it.h, u, w, true);
+      const uint32_t x0 = row_word(p, it.h, it.u0, w, true);
+      const uint32_t x1 = row_word(p, it.h, it.u0 + 1, w, it.has1);
+      uint32_t x = x0 | x1;
       while (x) {
-        const int j = w * 32 + (__ffs(x) - 1);
+        const int bit = __ffs(x) - 1;
         x &= x - 1u;
+        const uint32_t a = (x0 >> bit) & 1u, b = (x1 >> bit) & 1u;
+        const uint32_t my = wg + (t == 1 ? a : 0u);
+        wg += a + b;
+        if (!(t == 0 ? a : b)) continue;
+        const int j = w * 32 + bit;
+        const uint32_t buf = my & 1u, sel = nmine & 1u, par = (nmine >> 1) & 1u;
+        const uint32_t tm_s = tmem + lane_base + buf * 128;
         SA_TR(0);
-        mbar_wait(smem_u32(&ctl->s_full[t]), sp_phase, 21);
-        sp_phase ^= 1u;
+        mbar_wait(smem_u32(&ctl->s_full[t][sel]), par, 21);
         tc_fence_after();
         SA_TR(1);
         uint32_t sr[4][32];
@@ -430,6 +483,11 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t tmem, int t, i
             l_run *= alpha;
           }
           if (started) {                     // O_t holds earlier blocks: bring it to the new max
+            // PV(my-2) and older retired before S(my) was issued; PV(my-1) may still be in flight
+            if (prev_unit + 1u == my) {
+              mbar_wait(smem_u32(&ctl->pv_done[t][(nmine - 1u) & 1u]), ((nmine - 1u) >> 1) & 1u, 23);
+              tc_fence_after();
+            }
 #pragma unroll
             for (int cc = 0; cc < 4; ++cc) {
               uint32_t orr[32];
@@ -443,13 +501,16 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t tmem, int t, i
         }
         const float m_use = (m_run == -INFINITY) ? 0.f : m_run;
         SA_TR(3);
-        if (ragged) l_run += exp_tile<0>(sr, c, m_use, tm_s, ctl->p_full[t], lane);
-        else l_run += exp_tile<kPolyPairs>(sr, c, m_use, tm_s, ctl->p_full[t], lane);
+        if (ragged) l_run += exp_tile<0>(sr, c, m_use, tm_s, ctl->p_full[t][sel], lane);
+        else l_run += exp_tile<kPolyPairs>(sr, c, m_use, tm_s, ctl->p_full[t][sel], lane);
         SA_TR(4);
         started = true;
+        prev_unit = my;
+        ++nmine;
       }
     }
 
+    if (!exists) continue;
     // ---- epilogue: O / l -> bf16, lse = ln2 * (m + log2 l); empty row -> 0 / -inf
     const size_t grow = static_cast<size_t>(it.row0) + static_cast<size_t>(u) * kBlk + row;
     uint4* orow = reinterpret_cast<uint4*>(p.out + grow * kD);
@@ -486,7 +547,7 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t tmem, int t, i
   }
 #ifdef SA_TRACE
   if (lane == 0 && blockIdx.x < 2 && quarter == 0)
-    printf("trace cta %d wg %d blocks %lld: other+epi %lld | wait_s %lld | ld %lld | max+resc %lld | exp+st %lld (clk per block)\n",
+    printf("trace cta %d wg %d blocks %u: other+epi %u | wait_s %u | ld %u | max+resc %u | exp+st %u (clk per block)\n",
            blockIdx.x, t, tr_n, tr_acc[0] / tr_n, tr_acc[1] / tr_n, tr_acc[2] / tr_n, tr_acc[3] / tr_n, tr_acc[4] / tr_n);
 #endif
 }
@@ -513,9 +574,12 @@ fwd_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
       mbar_init(smem_u32(&ctl->kv_empty[s]), 1);
     }
     for (int t = 0; t < 2; ++t) {
-      mbar_init(smem_u32(&ctl->s_full[t]), 1);
-      for (int c = 0; c < 4; ++c)
-        mbar_init(smem_u32(&ctl->p_full[t][c]), 4);   // one arrival per softmax warp
+      for (int b = 0; b < 2; ++b) {
+        mbar_init(smem_u32(&ctl->s_full[t][b]), 1);
+        mbar_init(smem_u32(&ctl->pv_done[t][b]), 1);
+        for (int c = 0; c < 4; ++c)
+          mbar_init(smem_u32(&ctl->p_full[t][b][c]), 4);   // one arrival per softmax warp
+      }
       mbar_init(smem_u32(&ctl->o_full[t]), 1);
       mbar_init(smem_u32(&ctl->o_free[t]), 4);
     }

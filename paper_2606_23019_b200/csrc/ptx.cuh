@@ -48,7 +48,10 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
 // kWatchdogNs means a protocol bug: trap instead of hanging the GPU. (Everything is inlined: a
 // call here would force the register-heavy softmax warps to spill around it. Build with
 // -DSA_WATCHDOG_PRINT to have the watchdog say which wait timed out.)
-constexpr uint64_t kWatchdogNs = 10ull * 1000 * 1000 * 1000;
+#ifndef SA_WATCHDOG_NS
+#define SA_WATCHDOG_NS 10000000000ull
+#endif
+constexpr uint64_t kWatchdogNs = SA_WATCHDOG_NS;
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, int tag = 0) {
   if (mbar_try_wait(bar, parity)) return;
   const uint64_t t0 = globaltimer();
