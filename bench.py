@@ -203,6 +203,64 @@ def run_reference(args, rank: int, world: int) -> int:
 
 
 # ------------------------------------------------------------------ our arm
+def run_seq_grid(sa, dev, stream, peaks, H: int, log):
+    """the paper's own kernel experiment (Fig. 5 caption
+    PAPER.md:250) -- sequence length 1K..262K x density at block 128 -- plus a HunyuanVideo-shaped
+    layer. The paper compares with FlashAttention-3; here density 1 of the same
+    kernel is the reference. q, k, v ~ N(0,1) drawn on the device (seeded); masks are the
+    per-head top-fraction of i.i.d. U(0,1) block scores, diagonal on."""
+    import numpy as np
+    import torch
+    from paper_2606_23019_b200 import inputs
+    rows = []
+    shapes = [inputs.seq_grid_config(N, H) for N in inputs.SEQ_GRID_N] + [inputs.HUNYUAN]
+    for cfg in shapes:
+        g = torch.Generator(device=dev).manual_seed(cfg.qkv_seed)
+        q, k, v = [torch.randn((cfg.B, cfg.H, cfg.N, cfg.D), generator=g, device=dev,
+                               dtype=torch.float32).to(torch.bfloat16) for _ in range(3)]
+        out = torch.empty_like(q)
+        lse = torch.empty((cfg.B, cfg.H, cfg.N), dtype=torch.float32, device=dev)
+        ws = torch.empty(max(sa.sa_fwd_workspace_bytes(cfg.B, cfg.H, cfg.N, cfg.Bq), 256),
+                         dtype=torch.uint8, device=dev)
+        scores_np, _ = inputs.iid_block_scores(cfg, 1.0)
+        scores = torch.from_numpy(scores_np).to(dev)
+        t_dense = None
+        for d in inputs.SEQ_GRID_DENSITY:
+            dens_t = torch.full((cfg.H,), d, dtype=torch.float32, device=dev)
+            bits = sa.sa_pack_mask(scores, dens_t, True)
+            torch.cuda.synchronize()
+            nb = popcount_total(bits.cpu().numpy().view(np.uint32)) * cfg.B
+            reps = 3 if cfg.N >= 65536 and d >= 0.5 else 7
+            for _ in range(2):
+                sa.sa_block_sparse_attn_fwd_ex(q, k, v, bits, cfg.Bq, cfg.Bk, cfg.scale,
+                                               cfg.n_valid, out, lse, ws, stream)
+            torch.cuda.synchronize()
+            ts = []
+            for _ in range(reps):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                sa.sa_block_sparse_attn_fwd_ex(q, k, v, bits, cfg.Bq, cfg.Bk, cfg.scale,
+                                               cfg.n_valid, out, lse, ws, stream)
+                b.record(stream)
+                torch.cuda.synchronize()
+                ts.append(a.elapsed_time(b))
+            med = statistics.median(ts)
+            if d == 1.0:
+                t_dense = med
+            dens = nb / (cfg.B * cfg.H * cfg.NQB * cfg.NKB)
+            tf = effective_tflops(nb, cfg.flops_per_block(), med)
+            rows.append({"shape": cfg.name, "N": cfg.N, "H": cfg.H, "density": round(dens, 5),
+                         "ms_median": round(med, 4), "tflops": round(tf, 1),
+                         "frac_of_peak": round(tf / peaks["bf16_tflops"], 4),
+                         "speedup_vs_density1": round(t_dense / med, 3),
+                         "frac_of_ideal": round(t_dense / med * dens, 4)})
+            log(f"[bench] grid {cfg.name} density {dens:.4f}: {med:.4f} ms {tf:.1f} TFLOP/s "
+                f"speedup {t_dense / med:.2f} (ideal {1 / dens:.2f})")
+        del q, k, v, out, lse, scores
+        torch.cuda.empty_cache()
+    return rows
+
+
 def run_ours(args, rank: int, local_rank: int, world: int) -> int:
     import numpy as np
     import torch
@@ -364,6 +422,10 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> int:
             log(f"[bench] sweep {name}: density {dens:.4f} {med:.3f} ms {tf:.1f} TFLOP/s "
                 f"speedup {t_dense / med:.2f} (ideal {1 / dens:.2f})")
 
+    seq_grid = None
+    if rank == 0 and args.seqlen_grid:
+        seq_grid = run_seq_grid(sa, dev, stream, peaks, args.grid_heads, log)
+
     # ---- pack-mask kernel group on its own (HBM/ALU-bound; not the dominant kernel)
     pack_ms = None
     if rank == 0:
@@ -477,6 +539,7 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> int:
                 "peak_gbs": peaks["hbm_gbs"]},
             "cpu_baseline": cpu_baseline,
             "density_sweep": sweep,
+            "seqlen_grid": seq_grid,
         }
         print(json.dumps(line), flush=True)
     if dist is not None:
@@ -497,6 +560,10 @@ def main() -> int:
                     help="CPU time the cpu_baseline sample grows to (in 64-unit chunks)")
     ap.add_argument("--ref-rows-per-head", type=int, default=8)
     ap.add_argument("--no-sweep", action="store_true")
+    ap.add_argument("--seqlen-grid", action="store_true",
+                    help="also time the sequence-length x density grid (1K..262K tokens) and a "
+                         "HunyuanVideo-shaped layer; off by default to keep the default run short")
+    ap.add_argument("--grid-heads", type=int, default=12)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

@@ -197,3 +197,30 @@ def sample_units(row_popcount: np.ndarray, seed: int, n_heads: int = 8, n_random
                 seen.append(u)
         units += [(0, h, int(u)) for u in seen]
     return np.asarray(units, dtype=np.int32)
+
+
+# ---- second workload: the paper's own kernel experiment, a sequence-length
+# x sparsity grid at block 128 (Sec. 5.3, Fig. 5 caption PAPER.md:250; 1K..262K
+# tokens), plus a HunyuanVideo-shaped layer (33 frames x 1350 tokens = 44 550 tokens).
+# The paper gives no head count / head dim for it: H and D are parameters here.
+SEQ_GRID_N = (1024, 4096, 16384, 65536, 262144)
+SEQ_GRID_DENSITY = (1.0, 0.5, 0.25, 0.1, 0.05)
+
+
+def seq_grid_config(N: int, H: int, n_valid: Optional[int] = None, seed: int = 7) -> Config:
+    """One cell's shape: B=1, D=128, 128-blocks, no latent grid (masks are i.i.d., see
+    `iid_block_scores`)."""
+    return Config(f"grid-N{N}-H{H}", 1, H, N, 128, 128, 128, N if n_valid is None else n_valid,
+                  None, 1000 + seed, 2000 + seed, 0.0, 0.0)
+
+
+HUNYUAN = Config("hunyuan-33x1350", 1, 24, 44672, 128, 128, 128, 44550, None, 11, 111, 0.0, 0.0)
+
+
+def iid_block_scores(cfg: Config, density: float, seed: Optional[int] = None):
+    """Block scores ~ i.i.d. U(0,1) (seeded) with every head at `density`: their per-head
+    top-fraction is a uniformly random mask with exactly that density (diagonal forced by the
+    pack call). Returns (scores float32 [H][NQB][NKB], density float32 [H])."""
+    rng = np.random.Generator(np.random.PCG64(cfg.mask_seed if seed is None else seed))
+    scores = rng.random((cfg.H, cfg.NQB, cfg.NKB), dtype=np.float32)
+    return scores, np.full(cfg.H, float(density), dtype=np.float32)

@@ -339,6 +339,39 @@ def test_c5_adversarial_and_sparse_sweep_sampled_units(sa):
     _sampled_unit_parity(sa, cfg, q, k, v, bits, bits_t, variant=0, n_heads=2)
 
 
+def test_next1_262144_tokens_sampled_units(sa):
+    # the longest sequence of the paper's kernel experiment (262 144 tokens =
+    # 2048 key blocks = 64 mask words per row) at 5% density, ragged tail.
+    cfg = inputs.seq_grid_config(262144, H=2, n_valid=262144 - 37)
+    assert cfg.W == 64
+    q, k, v = inputs.make_qkv(cfg)
+    inputs.poison_padding(cfg, k, v)
+    scores, density = inputs.iid_block_scores(cfg, 0.05)
+    bits_t = sa.sa_pack_mask(torch.from_numpy(scores).cuda(), torch.from_numpy(density).cuda(),
+                             force_diag=True)
+    torch.cuda.synchronize()
+    bits = host_bits(bits_t)
+    assert (bits == oracle.pack_mask(scores, density, 1)).all()
+    _sampled_unit_parity(sa, cfg, q, k, v, bits, bits_t, variant=0, n_heads=2)
+
+
+@pytest.mark.parametrize("N", [1024, 4096])
+def test_next1_short_sequences_full_compare(sa, N):
+    # the short end of the grid (8 and 32 key blocks: fewer work items than SMs), full compare
+    cfg = inputs.seq_grid_config(N, H=3, seed=N)
+    q, k, v = inputs.make_qkv(cfg)
+    scores, density = inputs.iid_block_scores(cfg, 0.5)
+    bits_t = sa.sa_pack_mask(torch.from_numpy(scores).cuda(), torch.from_numpy(density).cuda(),
+                             force_diag=True)
+    torch.cuda.synchronize()
+    bits = host_bits(bits_t)
+    assert (bits == oracle.pack_mask(scores, density, 1)).all()
+    ref_o, ref_l = oracle.attn(inputs.as_u16(q), inputs.as_u16(k), inputs.as_u16(v), bits, 128, 128,
+                               cfg.scale)
+    out, lse = run_fwd(sa, q, k, v, bits, 128, cfg.scale)
+    check_out(out, lse, ref_o, ref_l, f"grid N={N}")
+
+
 def test_host_buffer_entry_point(sa):
     cfg = inputs.C1
     q, k, v = inputs.make_qkv(cfg, pin_memory=True)
