@@ -438,6 +438,29 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> int:
         torch.cuda.synchronize()
         pack_ms = a.elapsed_time(b) / 10
 
+    # ---- the paper's run-time mask path on its own: a threshold map at the
+    # 480p block grid (256 x 256) instantiated at this workload's grid, Eq. 7
+    thr = None
+    if rank == 0:
+        nb_base = 256
+        tmap = torch.rand((cfg.H, nb_base, nb_base), device=dev, dtype=torch.float32)
+        p_star = torch.full((cfg.H,), 0.2, device=dev, dtype=torch.float32)
+        bits_thr = torch.empty_like(bits)
+        sa.sa_mask_from_threshold(tmap, p_star, cfg.NQB, cfg.NKB, True, bits_thr, stream)
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(10):
+            sa.sa_mask_from_threshold(tmap, p_star, cfg.NQB, cfg.NKB, True, bits_thr, stream)
+        b.record(stream)
+        torch.cuda.synchronize()
+        thr_ms = a.elapsed_time(b) / 10
+        thr_bytes = tmap.numel() * 4 + bits_thr.numel() * 4
+        thr = {"ms": thr_ms, "bound": "hbm", "base_grid": [nb_base, nb_base],
+               "target_grid": [cfg.NQB, cfg.NKB], "algorithmic_bytes": thr_bytes,
+               "achieved_gbs": thr_bytes / (thr_ms * 1e-3) / 1e9, "peak_gbs": peaks["hbm_gbs"]}
+        del tmap, bits_thr
+
     # ---- CPU baseline: the oracle, as it stands, on a bounded sample of the same workload
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -537,6 +560,7 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> int:
                 "algorithmic_bytes": scores.numel() * 4 + bits.numel() * 4,
                 "achieved_gbs": (scores.numel() * 4 + bits.numel() * 4) / (pack_ms * 1e-3) / 1e9,
                 "peak_gbs": peaks["hbm_gbs"]},
+            "mask_from_threshold": thr,
             "cpu_baseline": cpu_baseline,
             "density_sweep": sweep,
             "seqlen_grid": seq_grid,

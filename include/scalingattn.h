@@ -72,6 +72,23 @@ SA_API sa_status sa_pack_mask(const float* scores, const float* density, uint32_
                        int NQB, int NKB, int force_diag, void* workspace, size_t workspace_bytes,
                        void* stream);
 
+/* The paper's run-time mask path: a per-head THRESHOLD MAP kept at a base resolution, instantiated
+ * at the target resolution (PAPER.md:103 M_p = 1(T <= p); Eq. 7, the conservative
+ * bilinear resize with a ceiling rule; readings P14-P16):
+ *   R_base[h][a][b]  = 1 if tmap[h][a][b] <= p_star[h] else 0              (fp32 comparison)
+ *   bit (u,v) of head h = ceil( Phi(R_base[h], u*nbq/NQB, v*nbk/NKB) )     (Phi = bilinear, no
+ *             half-cell offset, neighbours clamped to the last cell): on exactly when a base cell
+ *             with positive interpolation weight is on. nbq == NQB and nbk == NKB gives 1(T <= p).
+ *   force_diag != 0 additionally sets every bit (u,u).
+ *   tmap    : fp32 [H][nbq][nbk] row-major (device);  p_star : fp32 [H] (device)
+ *   mask_bits (out): uint32 [H][NQB][W], W = ceil(NKB/32), bits at positions >= NKB written 0.
+ * Bit-exact and deterministic (integer index arithmetic only); one kernel on `stream`, no workspace,
+ * no synchronisation. SA_ERR_INVALID_ARG for null / misaligned (16 B) pointers or non-positive sizes;
+ * SA_ERR_UNSUPPORTED if a grid side exceeds 32768 blocks. */
+SA_API sa_status sa_mask_from_threshold(const float* tmap, const float* p_star, uint32_t* mask_bits,
+                                        int H, int nbq, int nbk, int NQB, int NKB, int force_diag,
+                                        void* stream);
+
 /* Block-sparse attention forward (Sec. 4.3.2; Alg. 2):
  *   out[b,h,i,:] = sum_j softmax_j(scale * <q[b,h,i,:], k[b,h,j,:]>) * v[b,h,j,:]
  *   lse[b,h,i]   = ln sum_j exp(scale * <q_i, k_j>)                       (natural log)

@@ -51,6 +51,8 @@ def load_library() -> C.CDLL:
     lib.sa_fwd_host_scratch_bytes.argtypes = [ip] * 6
     lib.sa_pack_mask.restype = ip
     lib.sa_pack_mask.argtypes = [vp, vp, vp, ip, ip, ip, ip, vp, sz, vp]
+    lib.sa_mask_from_threshold.restype = ip
+    lib.sa_mask_from_threshold.argtypes = [vp, vp, vp, ip, ip, ip, ip, ip, ip, vp]
     lib.sa_block_sparse_attn_fwd.restype = ip
     lib.sa_block_sparse_attn_fwd.argtypes = [vp, vp, vp, vp, vp, vp, ip, ip, ip, ip, ip, ip, fp, vp]
     lib.sa_block_sparse_attn_fwd_ex.restype = ip
@@ -151,6 +153,23 @@ def sa_pack_mask(scores, density, force_diag: bool = True, mask_bits=None, works
     _check(lib.sa_pack_mask(_ptr(scores), _ptr(density), _ptr(mask_bits), H, NQB, NKB,
                             int(bool(force_diag)), _ptr(workspace), workspace.numel(),
                             _stream(stream)))
+    return mask_bits
+
+
+def sa_mask_from_threshold(tmap, p_star, NQB: int, NKB: int, force_diag: bool = True,
+                           mask_bits=None, stream=None):
+    """tmap fp32 [H][nbq][nbk], p_star fp32 [H] (device) -> mask_bits int32 [H][NQB][W] (uint32 bit
+    patterns): 1(T <= p*) at the base resolution, conservatively resized to NQB x NKB (Eq. 7)."""
+    lib = load_library()
+    assert tmap.dtype == torch.float32 and tmap.is_contiguous() and tmap.dim() == 3
+    assert p_star.dtype == torch.float32 and p_star.is_contiguous()
+    H, nbq, nbk = tmap.shape
+    assert p_star.shape == (H,)
+    W = (NKB + 31) // 32
+    if mask_bits is None:
+        mask_bits = torch.empty((H, NQB, W), dtype=torch.int32, device=tmap.device)
+    _check(lib.sa_mask_from_threshold(_ptr(tmap), _ptr(p_star), _ptr(mask_bits), H, nbq, nbk,
+                                      int(NQB), int(NKB), int(bool(force_diag)), _stream(stream)))
     return mask_bits
 
 

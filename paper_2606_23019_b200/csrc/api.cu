@@ -145,6 +145,31 @@ sa_status sa_pack_mask(const float* scores, const float* density, uint32_t* mask
   return SA_OK;
 }
 
+sa_status sa_mask_from_threshold(const float* tmap, const float* p_star, uint32_t* mask_bits, int H,
+                                 int nbq, int nbk, int NQB, int NKB, int force_diag, void* stream) {
+  g_last_launches = 0;
+  if (!tmap || !p_star || !mask_bits)
+    return fail(SA_ERR_INVALID_ARG, "sa_mask_from_threshold: null pointer");
+  if (H <= 0 || nbq <= 0 || nbk <= 0 || NQB <= 0 || NKB <= 0)
+    return fail(SA_ERR_INVALID_ARG,
+                "sa_mask_from_threshold: sizes must be positive (H=%d nbq=%d nbk=%d NQB=%d NKB=%d)", H,
+                nbq, nbk, NQB, NKB);
+  if (!aligned16(tmap) || !aligned16(mask_bits))
+    return fail(SA_ERR_INVALID_ARG, "sa_mask_from_threshold: pointers must be 16-byte aligned");
+  if (nbq > 32768 || nbk > 32768 || NQB > 32768 || NKB > 32768 ||
+      static_cast<long long>(H) * NQB * ((NKB + 31) / 32) > 0x3FFFFFFFLL)
+    return fail(SA_ERR_UNSUPPORTED,
+                "sa_mask_from_threshold: a grid side exceeds 32768 blocks or the mask 2^30 words");
+  sa_status s = check_device();
+  if (s != SA_OK) return s;
+  cudaError_t e = sa::launch_mask_from_threshold(tmap, p_star, mask_bits, H, nbq, nbk, NQB, NKB,
+                                                 force_diag ? 1 : 0,
+                                                 static_cast<cudaStream_t>(stream));
+  if (e != cudaSuccess) return cuda_fail(e, "sa_mask_from_threshold launch");
+  g_last_launches = 1;
+  return SA_OK;
+}
+
 sa_status sa_block_sparse_attn_fwd_ex(const void* q, const void* k, const void* v,
                                       const uint32_t* mask_bits, void* out, float* lse, int B,
                                       int H, int N, int n_valid, int D, int Bq, int Bk,

@@ -9,6 +9,7 @@ import pytest
 import torch
 
 import oracle
+from oracle import threshold as oracle_threshold
 from paper_2606_23019_b200 import inputs
 
 pytestmark = pytest.mark.gpu
@@ -370,6 +371,58 @@ def test_next1_short_sequences_full_compare(sa, N):
                                cfg.scale)
     out, lse = run_fwd(sa, q, k, v, bits, 128, cfg.scale)
     check_out(out, lse, ref_o, ref_l, f"grid N={N}")
+
+
+# ------------------------------------------------------------------ NEXT-2: mask from a threshold map
+def _threshold_map(H, nbq, nbk, seed):
+    rng = np.random.Generator(np.random.PCG64(seed))
+    # discrete levels like the paper's candidate set; many ties with p* on purpose
+    return (rng.integers(1, 49, size=(H, nbq, nbk)) / 48.0).astype(np.float32)
+
+
+@pytest.mark.parametrize("nbq,nbk,NQB,NKB,force_diag", [
+    (16, 16, 16, 16, 1), (7, 45, 7, 45, 0), (5, 7, 12, 9, 0), (8, 8, 5, 3, 0), (6, 6, 6, 13, 0),
+    (1, 1, 4, 4, 1), (16, 16, 37, 37, 1), (33, 33, 64, 64, 1), (40, 31, 97, 65, 0)])
+def test_mask_from_threshold_bit_exact(sa, nbq, nbk, NQB, NKB, force_diag):
+    H = 3
+    T = _threshold_map(H, nbq, nbk, nbq * 1000 + NQB)
+    p = np.array([0.25, 0.5, 11 / 48.0], dtype=np.float32)
+    ref = oracle.pack_bool(oracle_threshold.mask_from_threshold(T, p, NQB, NKB, bool(force_diag)))
+    got = host_bits(sa.sa_mask_from_threshold(torch.from_numpy(T).cuda(), torch.from_numpy(p).cuda(),
+                                              NQB, NKB, force_diag=bool(force_diag)))
+    assert got.shape == ref.shape and (got == ref).all()
+
+
+def test_mask_from_threshold_480p_to_720p_then_attention(sa):
+    # the paper's deployment path: a map built at the 480p block grid (256 x 256) reused at the 720p
+    # one (591 x 591), then consumed by the forward pass; sampled rows of the
+    # resized mask against the oracle (the full 591 x 591 x H loop is slow in pure Python), then
+    # sampled attention units at 720p shapes with 2 heads.
+    cfg = inputs.scaled(inputs.C4, H=2)
+    base = inputs.scaled(inputs.C2, H=2)
+    scores, _, _ = inputs.make_block_scores(base)
+    # a threshold map from the structured scores: rank of each block within its head, as a fraction
+    order = np.argsort(np.argsort(-scores.reshape(2, -1), axis=1, kind="stable"), axis=1, kind="stable")
+    T = ((order + 1) / float(base.NQB * base.NKB)).astype(np.float32).reshape(2, base.NQB, base.NKB)
+    p = np.array([0.15, 0.3], dtype=np.float32)
+    bits_t = sa.sa_mask_from_threshold(torch.from_numpy(T).cuda(), torch.from_numpy(p).cuda(),
+                                       cfg.NQB, cfg.NKB, force_diag=True)
+    torch.cuda.synchronize()
+    bits = host_bits(bits_t)
+    dense = oracle.unpack_mask(bits, cfg.NKB)
+    rng = np.random.Generator(np.random.PCG64(8))
+    for h in range(2):
+        R = oracle_threshold.mask_at(T[h], p[h])
+        for u in [0, 1, cfg.NQB - 1] + rng.integers(0, cfg.NQB, size=5).tolist():
+            x = (u * base.NQB) / cfg.NQB
+            row = [1 if (u == v or np.ceil(oracle_threshold.phi(R, x, (v * base.NKB) / cfg.NKB)) > 0) else 0
+                   for v in range(cfg.NKB)]
+            assert dense[h, u].tolist() == row
+    # conservative: the density can only grow, and by less than the 2x2 support allows
+    assert dense[0].mean() >= 0.15 and dense[1].mean() >= 0.3 and dense.mean() < 0.6
+    q, k, v = inputs.make_qkv(cfg)
+    inputs.poison_padding(cfg, k, v)
+    _sampled_unit_parity(sa, cfg, q, k, v, bits, bits_t, variant=0, n_heads=2)
 
 
 def test_host_buffer_entry_point(sa):
