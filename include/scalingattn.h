@@ -89,6 +89,23 @@ SA_API sa_status sa_mask_from_threshold(const float* tmap, const float* p_star, 
                                         int H, int nbq, int nbk, int NQB, int NKB, int force_diag,
                                         void* stream);
 
+/* FAST's Fidelity Score from the forward pass's log-sum-exp (Eq. 3 Hellinger distance,
+ * PAPER.md:132-134 Eq. 4 F = 1 - H, PAPER.md:155-159 stratified row sample; reading P17):
+ * with P the dense softmax row and P~ the softmax over the kept keys only,
+ *   H(P, P~) = sqrt(1 - sqrt(rho)),  rho = exp(lse_sparse - lse_dense) = retained attention mass,
+ * so for every (b,h):  fidelity[b][h] = mean over i < n_rows of 1 - H at query row rows[i].
+ *   lse_dense, lse_sparse : fp32 [B][H][N] (device), the lse outputs of two forward calls on the same
+ *                           q, k, scale, n_valid: all-ones mask and the candidate mask
+ *   rows        : int32 [n_rows] (device), query-row indices in [0, N), drawn by the caller (e.g. a few
+ *                 per row block, Sec. 4.2.3), shared by all (b,h); an index outside [0, N) makes the
+ *                 affected outputs NaN
+ *   fidelity    : fp32 [B][H] (out);   per_row : fp32 [B][H][n_rows] (out) or NULL
+ * A row empty in both masks scores 1, a row whose kept set is empty scores 0. Deterministic. One kernel
+ * on `stream`, no workspace, no synchronisation. */
+SA_API sa_status sa_fidelity_from_lse(const float* lse_dense, const float* lse_sparse,
+                                      const int32_t* rows, int n_rows, int B, int H, int N,
+                                      float* fidelity, float* per_row, void* stream);
+
 /* Block-sparse attention forward (Sec. 4.3.2; Alg. 2):
  *   out[b,h,i,:] = sum_j softmax_j(scale * <q[b,h,i,:], k[b,h,j,:]>) * v[b,h,j,:]
  *   lse[b,h,i]   = ln sum_j exp(scale * <q_i, k_j>)                       (natural log)

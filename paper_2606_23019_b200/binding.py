@@ -53,6 +53,8 @@ def load_library() -> C.CDLL:
     lib.sa_pack_mask.argtypes = [vp, vp, vp, ip, ip, ip, ip, vp, sz, vp]
     lib.sa_mask_from_threshold.restype = ip
     lib.sa_mask_from_threshold.argtypes = [vp, vp, vp, ip, ip, ip, ip, ip, ip, vp]
+    lib.sa_fidelity_from_lse.restype = ip
+    lib.sa_fidelity_from_lse.argtypes = [vp, vp, vp, ip, ip, ip, ip, vp, vp, vp]
     lib.sa_block_sparse_attn_fwd.restype = ip
     lib.sa_block_sparse_attn_fwd.argtypes = [vp, vp, vp, vp, vp, vp, ip, ip, ip, ip, ip, ip, fp, vp]
     lib.sa_block_sparse_attn_fwd_ex.restype = ip
@@ -171,6 +173,22 @@ def sa_mask_from_threshold(tmap, p_star, NQB: int, NKB: int, force_diag: bool = 
     _check(lib.sa_mask_from_threshold(_ptr(tmap), _ptr(p_star), _ptr(mask_bits), H, nbq, nbk,
                                       int(NQB), int(NKB), int(bool(force_diag)), _stream(stream)))
     return mask_bits
+
+
+def sa_fidelity_from_lse(lse_dense, lse_sparse, rows, per_row: bool = False, stream=None):
+    """lse_dense, lse_sparse fp32 [B][H][N], rows int32 [n_rows] (device) -> fidelity fp32 [B][H]
+    (and the per-row scores fp32 [B][H][n_rows] if per_row)."""
+    lib = load_library()
+    assert lse_dense.dtype == lse_sparse.dtype == torch.float32 and lse_dense.shape == lse_sparse.shape
+    assert lse_dense.is_contiguous() and lse_sparse.is_contiguous() and lse_dense.dim() == 3
+    assert rows.dtype == torch.int32 and rows.is_contiguous() and rows.dim() == 1
+    B, H, N = lse_dense.shape
+    fid = torch.empty((B, H), dtype=torch.float32, device=lse_dense.device)
+    pr = (torch.empty((B, H, rows.numel()), dtype=torch.float32, device=lse_dense.device)
+          if per_row else None)
+    _check(lib.sa_fidelity_from_lse(_ptr(lse_dense), _ptr(lse_sparse), _ptr(rows), rows.numel(), B, H,
+                                    N, _ptr(fid), _ptr(pr), _stream(stream)))
+    return (fid, pr) if per_row else fid
 
 
 def _fwd_shapes(q, k, v, mask_bits, Bq, Bk):

@@ -170,6 +170,26 @@ sa_status sa_mask_from_threshold(const float* tmap, const float* p_star, uint32_
   return SA_OK;
 }
 
+sa_status sa_fidelity_from_lse(const float* lse_dense, const float* lse_sparse, const int32_t* rows,
+                               int n_rows, int B, int H, int N, float* fidelity, float* per_row,
+                               void* stream) {
+  g_last_launches = 0;
+  if (!lse_dense || !lse_sparse || !rows || !fidelity)
+    return fail(SA_ERR_INVALID_ARG, "sa_fidelity_from_lse: null pointer");
+  if (n_rows <= 0 || B <= 0 || H <= 0 || N <= 0)
+    return fail(SA_ERR_INVALID_ARG, "sa_fidelity_from_lse: sizes must be positive (n_rows=%d B=%d H=%d N=%d)",
+                n_rows, B, H, N);
+  if (static_cast<long long>(B) * H > 0x7FFFFFFFLL)
+    return fail(SA_ERR_UNSUPPORTED, "sa_fidelity_from_lse: B*H exceeds 2^31-1");
+  sa_status s = check_device();
+  if (s != SA_OK) return s;
+  cudaError_t e = sa::launch_fidelity(lse_dense, lse_sparse, rows, n_rows, B * H, N, fidelity, per_row,
+                                      static_cast<cudaStream_t>(stream));
+  if (e != cudaSuccess) return cuda_fail(e, "sa_fidelity_from_lse launch");
+  g_last_launches = 1;
+  return SA_OK;
+}
+
 sa_status sa_block_sparse_attn_fwd_ex(const void* q, const void* k, const void* v,
                                       const uint32_t* mask_bits, void* out, float* lse, int B,
                                       int H, int N, int n_valid, int D, int Bq, int Bk,

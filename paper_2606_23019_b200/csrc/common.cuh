@@ -93,6 +93,9 @@ constexpr int kPackMaskLaunches = 6;   // kernels launch_pack_mask enqueues (plu
 cudaError_t launch_mask_from_threshold(const float* tmap, const float* p_star, uint32_t* mask_bits,
                                        int H, int nbq, int nbk, int NQB, int NKB, int force_diag,
                                        cudaStream_t st);
+cudaError_t launch_fidelity(const float* lse_dense, const float* lse_sparse, const int32_t* rows,
+                            int n_rows, int BH, int N, float* fidelity, float* per_row,
+                            cudaStream_t st);
 cudaError_t launch_enumerate(const uint32_t* mask_bits, int H, int NQB, int NKB, int32_t* idx,
                              int32_t* cnt, cudaStream_t st);
 

@@ -10,6 +10,7 @@ import torch
 
 import oracle
 from oracle import threshold as oracle_threshold
+from oracle import fidelity as oracle_fidelity
 from paper_2606_23019_b200 import inputs
 
 pytestmark = pytest.mark.gpu
@@ -423,6 +424,46 @@ def test_mask_from_threshold_480p_to_720p_then_attention(sa):
     q, k, v = inputs.make_qkv(cfg)
     inputs.poison_padding(cfg, k, v)
     _sampled_unit_parity(sa, cfg, q, k, v, bits, bits_t, variant=0, n_heads=2)
+
+
+# ------------------------------------------------------------------ NEXT-4: fidelity from LSE
+def test_fidelity_from_lse_matches_hellinger_definition(sa):
+    # F = 1 - H(P, P~) (Eq. 3-4) on a stratified row sample (2 rows per query block, Sec. 4.2.3):
+    # the CUDA path gets it from the lse of two forward calls; the oracle builds both distributions
+    # explicitly and applies the definition. Head 0: random 40% mask, head 1: all ones (F == 1
+    # exactly), head 2: diagonal only. Ragged tail (n_valid < N).
+    D, blk, H, nblk = 128, 128, 3, 10
+    N, n_valid = nblk * blk, nblk * blk - 50
+    q, k, v, m = _small_case(D, blk, H, nblk, seed=21)
+    m[1] = True
+    m[2] = np.eye(nblk, dtype=bool)
+    bits_s = oracle.pack_bool(m)
+    bits_d = oracle.pack_bool(np.ones_like(m))
+    scale = float(np.float32(1 / math.sqrt(D)))
+    _, lse_d = run_fwd(sa, q, k, v, bits_d, blk, scale, n_valid=n_valid)
+    _, lse_s = run_fwd(sa, q, k, v, bits_s, blk, scale, n_valid=n_valid)
+    rng = np.random.Generator(np.random.PCG64(22))
+    rows = np.concatenate([u * blk + rng.choice(blk, size=2, replace=False) for u in range(nblk)])
+    rows = rows.astype(np.int32)
+    fid, per_row = sa.sa_fidelity_from_lse(lse_d, lse_s, torch.from_numpy(rows).cuda(), per_row=True)
+    torch.cuda.synchronize()
+    fid, per_row = fid.cpu().numpy(), per_row.cpu().numpy()
+    qa, ka, va = inputs.as_u16(q), inputs.as_u16(k), inputs.as_u16(v)
+    for h in range(H):
+        ref = []
+        for i in rows.tolist():
+            Pd, _, _ = oracle.attn_row_weights(qa, ka, va, bits_d, blk, blk, scale, 0, h, i, n_valid=n_valid)
+            Ps, _, _ = oracle.attn_row_weights(qa, ka, va, bits_s, blk, blk, scale, 0, h, i, n_valid=n_valid)
+            ref.append(oracle_fidelity.fidelity(Pd, Ps))
+        ref = np.asarray(ref)
+        # fp32 lse carries ~1e-5 absolute error and dH = d(lse) / (4 H): 5e-3 covers H down to 1e-3
+        assert np.abs(per_row[0, h] - ref).max() <= 5e-3, (h, np.abs(per_row[0, h] - ref).max())
+        assert abs(fid[0, h] - ref.mean()) <= 2e-3
+    assert fid[0, 1] == 1.0                       # the dense head loses nothing
+    assert fid[0, 2] < fid[0, 0] < 1.0            # diagonal-only keeps less mass than the 40% mask
+    # a row index outside [0, N) poisons the result instead of reading out of bounds
+    bad = sa.sa_fidelity_from_lse(lse_d, lse_s, torch.tensor([0, N], dtype=torch.int32).cuda())
+    assert torch.isnan(bad).all()
 
 
 def test_host_buffer_entry_point(sa):
