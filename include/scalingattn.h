@@ -89,6 +89,20 @@ SA_API sa_status sa_mask_from_threshold(const float* tmap, const float* p_star, 
                                         int H, int nbq, int nbk, int NQB, int NKB, int force_diag,
                                         void* stream);
 
+/* WEST's block-wise aggregation (Eq. 1; Alg. 1 l.9-10 PAPER.md:396-398) without
+ * materialising the attention matrix: with lse the output of a forward call on the all-ones mask,
+ *   sig[b][h][u][v] = (1/(Bq*Bk)) * sum_{i in block u, i < n_valid} sum_{j in block v, j < n_valid}
+ *                     exp(scale * <q[b,h,i,:], k[b,h,j,:]> - lse[b,h,i])
+ * (each valid query row spreads mass 1 over the key blocks; padded rows are left out, padded keys get
+ * zero weight: DESIGN.md P18). A batch entry is one calibration sample.
+ *   q, k : bf16 [B][H][N][D] (device, 16 B aligned);  lse : fp32 [B][H][N] (device)
+ *   sig  : fp32 [B][H][N/Bq][N/Bk] (out, device)
+ * Supported: (D,Bq,Bk) = (128,128,128) on sm_100 (SA_ERR_UNSUPPORTED otherwise). Deterministic. One
+ * tcgen05 kernel on `stream`, no workspace, no synchronisation. */
+SA_API sa_status sa_block_significance(const void* q, const void* k, const float* lse, float* sig,
+                                       int B, int H, int N, int n_valid, int D, int Bq, int Bk,
+                                       float scale, void* stream);
+
 /* FAST's Fidelity Score from the forward pass's log-sum-exp (Eq. 3 Hellinger distance,
  * PAPER.md:132-134 Eq. 4 F = 1 - H, PAPER.md:155-159 stratified row sample; reading P17):
  * with P the dense softmax row and P~ the softmax over the kept keys only,

@@ -53,6 +53,8 @@ def load_library() -> C.CDLL:
     lib.sa_pack_mask.argtypes = [vp, vp, vp, ip, ip, ip, ip, vp, sz, vp]
     lib.sa_mask_from_threshold.restype = ip
     lib.sa_mask_from_threshold.argtypes = [vp, vp, vp, ip, ip, ip, ip, ip, ip, vp]
+    lib.sa_block_significance.restype = ip
+    lib.sa_block_significance.argtypes = [vp, vp, vp, vp, ip, ip, ip, ip, ip, ip, ip, fp, vp]
     lib.sa_fidelity_from_lse.restype = ip
     lib.sa_fidelity_from_lse.argtypes = [vp, vp, vp, ip, ip, ip, ip, vp, vp, vp]
     lib.sa_block_sparse_attn_fwd.restype = ip
@@ -173,6 +175,23 @@ def sa_mask_from_threshold(tmap, p_star, NQB: int, NKB: int, force_diag: bool = 
     _check(lib.sa_mask_from_threshold(_ptr(tmap), _ptr(p_star), _ptr(mask_bits), H, nbq, nbk,
                                       int(NQB), int(NKB), int(bool(force_diag)), _stream(stream)))
     return mask_bits
+
+
+def sa_block_significance(q, k, lse, Bq: int, Bk: int, scale: float, n_valid=None, sig=None,
+                          stream=None):
+    """q, k bf16 [B][H][N][D], lse fp32 [B][H][N] (of a dense forward call) -> block significance
+    fp32 [B][H][N/Bq][N/Bk] (Eq. 1)."""
+    lib = load_library()
+    assert q.dtype == k.dtype == torch.bfloat16 and q.is_contiguous() and k.is_contiguous()
+    assert q.shape == k.shape and q.dim() == 4
+    B, H, N, D = q.shape
+    assert lse.dtype == torch.float32 and tuple(lse.shape) == (B, H, N) and lse.is_contiguous()
+    n_valid = N if n_valid is None else int(n_valid)
+    if sig is None:
+        sig = torch.empty((B, H, N // Bq, N // Bk), dtype=torch.float32, device=q.device)
+    _check(lib.sa_block_significance(_ptr(q), _ptr(k), _ptr(lse), _ptr(sig), B, H, N, n_valid, D, Bq,
+                                     Bk, float(scale), _stream(stream)))
+    return sig
 
 
 def sa_fidelity_from_lse(lse_dense, lse_sparse, rows, per_row: bool = False, stream=None):

@@ -170,6 +170,27 @@ sa_status sa_mask_from_threshold(const float* tmap, const float* p_star, uint32_
   return SA_OK;
 }
 
+sa_status sa_block_significance(const void* q, const void* k, const float* lse, float* sig, int B,
+                                int H, int N, int n_valid, int D, int Bq, int Bk, float scale,
+                                void* stream) {
+  g_last_launches = 0;
+  if (!q || !k || !lse || !sig) return fail(SA_ERR_INVALID_ARG, "sa_block_significance: null pointer");
+  sa_status s = validate_shape(B, H, N, n_valid, D, Bq, Bk, scale);
+  if (s != SA_OK) return s;
+  if (D != 128) return fail(SA_ERR_UNSUPPORTED, "sa_block_significance: only (D,Bq,Bk) = (128,128,128)");
+  if (!aligned16(q) || !aligned16(k))
+    return fail(SA_ERR_INVALID_ARG, "sa_block_significance: q, k must be 16-byte aligned");
+  s = check_device();
+  if (s != SA_OK) return s;
+  const char* txt = nullptr;
+  cudaError_t e = sa::launch_block_significance(static_cast<const __nv_bfloat16*>(q),
+                                                static_cast<const __nv_bfloat16*>(k), lse, sig, B, H, N,
+                                                n_valid, scale, static_cast<cudaStream_t>(stream), &txt);
+  if (e != cudaSuccess) return cuda_fail(e, txt ? txt : "sa_block_significance launch");
+  g_last_launches = 1;
+  return SA_OK;
+}
+
 sa_status sa_fidelity_from_lse(const float* lse_dense, const float* lse_sparse, const int32_t* rows,
                                int n_rows, int B, int H, int N, float* fidelity, float* per_row,
                                void* stream) {

@@ -93,6 +93,10 @@ constexpr int kPackMaskLaunches = 6;   // kernels launch_pack_mask enqueues (plu
 cudaError_t launch_mask_from_threshold(const float* tmap, const float* p_star, uint32_t* mask_bits,
                                        int H, int nbq, int nbk, int NQB, int NKB, int force_diag,
                                        cudaStream_t st);
+bool make_tile_map_128x64(void* map /* CUtensorMap* */, const void* base, uint64_t rows);
+cudaError_t launch_block_significance(const __nv_bfloat16* q, const __nv_bfloat16* k, const float* lse,
+                                      float* sig, int B, int H, int N, int n_valid, float scale,
+                                      cudaStream_t st, const char** err_text);
 cudaError_t launch_fidelity(const float* lse_dense, const float* lse_sparse, const int32_t* rows,
                             int n_rows, int BH, int N, float* fidelity, float* per_row,
                             cudaStream_t st);

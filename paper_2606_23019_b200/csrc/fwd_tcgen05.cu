@@ -647,6 +647,11 @@ bool make_map(CUtensorMap* m, const void* base, uint64_t rows) {
 
 }  // namespace
 
+// shared with sig_tcgen05.cu: CUtensorMap of a [rows][128] bf16 array, box 64 x 128, 128B swizzle
+bool make_tile_map_128x64(void* map, const void* base, uint64_t rows) {
+  return make_map(static_cast<CUtensorMap*>(map), base, rows);
+}
+
 cudaError_t launch_fwd_tcgen05(const FwdParams& p, void*, cudaStream_t st, int* n_launch,
                                const char** err_text) {
   static int n_sm = 0;

@@ -11,6 +11,7 @@ import torch
 import oracle
 from oracle import threshold as oracle_threshold
 from oracle import fidelity as oracle_fidelity
+from oracle import west as oracle_west
 from paper_2606_23019_b200 import inputs
 
 pytestmark = pytest.mark.gpu
@@ -464,6 +465,35 @@ def test_fidelity_from_lse_matches_hellinger_definition(sa):
     # a row index outside [0, N) poisons the result instead of reading out of bounds
     bad = sa.sa_fidelity_from_lse(lse_d, lse_s, torch.tensor([0, N], dtype=torch.int32).cuda())
     assert torch.isnan(bad).all()
+
+
+# ------------------------------------------------------------------ NEXT-3: WEST block aggregation
+def test_block_significance_matches_eq1(sa):
+    # Eq. 1 from the lse of a dense forward call vs the oracle's explicit softmax + block mean.
+    # 11 key blocks (odd: the two S buffers swap roles between items), ragged tail, B = 2 samples,
+    # scores with some spread so that block sums differ by orders of magnitude.
+    D, blk, H, nblk = 128, 128, 3, 11
+    N, n_valid = nblk * blk, nblk * blk - 70
+    g = torch.Generator().manual_seed(31)
+    q = (torch.randn((2, H, N, D), generator=g) * 2).to(torch.bfloat16)
+    k = torch.randn((2, H, N, D), generator=g).to(torch.bfloat16)
+    v = torch.randn((2, H, N, D), generator=g).to(torch.bfloat16)
+    scale = float(np.float32(1 / math.sqrt(D)))
+    ones = oracle.pack_bool(np.ones((H, nblk, nblk), dtype=bool))
+    _, lse = run_fwd(sa, q, k, v, ones, blk, scale, n_valid=n_valid)
+    sig = sa.sa_block_significance(q.cuda(), k.cuda(), lse, blk, blk, scale, n_valid=n_valid)
+    torch.cuda.synchronize()
+    sig = sig.cpu().numpy().astype(np.float64)
+    for b in range(2):
+        for h in range(H):
+            ref = oracle_west.block_significance(q[b, h].float().numpy(), k[b, h].float().numpy(), scale,
+                                                 blk, n_valid)
+            # bf16 inputs are exact on both sides; ex2.approx, fp32 sums and the fp32 lse (~1e-5) leave
+            # ~1e-4 relative on a block sum
+            err = np.abs(sig[b, h] - ref)
+            assert (err <= 1e-3 * ref + 1e-12).all(), (b, h, (err / (ref + 1e-30)).max())
+            rows = np.minimum(np.maximum(n_valid - np.arange(nblk) * blk, 0), blk)
+            assert np.abs(sig[b, h].sum(axis=1) - rows / (blk * blk)).max() < 1e-6   # row mass
 
 
 def test_host_buffer_entry_point(sa):
