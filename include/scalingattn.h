@@ -103,6 +103,23 @@ SA_API sa_status sa_block_significance(const void* q, const void* k, const float
                                        int B, int H, int N, int n_valid, int D, int Bq, int Bk,
                                        float scale, void* stream);
 
+/* WEST's local threshold discovery and topology union (Alg. 1 l.12-17; DESIGN.md
+ * readings P19-P20) for a batch of calibration samples. For every sample b and head h: sort the block
+ * significances sig[b][h] in descending order (ties in flat-index order), C = inclusive cumulative sum
+ * divided by its total; the blocks at sorted positions 0..tau(p) are active at level p, tau(p) the first
+ * position with C >= p; L(u,v) = the smallest level at which (u,v) is active, 1.0 if none; then
+ *   tmap[h][u][v] <- min(tmap[h][u][v], L(u,v))        (union over the samples of the batch).
+ *   sig    : fp32 [B][H][NQB][NKB] (device), non-negative, e.g. from sa_block_significance
+ *   levels : fp32 [n_levels] (device), ascending, in (0, 1], n_levels <= 256 (the candidate set P)
+ *   tmap   : fp32 [H][NQB][NKB] (device, in/out); initialise with 1.0 before the first sample
+ *   workspace >= sa_threshold_map_update_workspace_bytes(B,H,NQB,NKB) bytes, 256 B aligned.
+ * The sort is cub::DeviceSegmentedRadixSort; everything runs on `stream` without synchronising.
+ * Deterministic. SA_ERR_UNSUPPORTED if B*H*NQB*NKB >= 2^31 or n_levels > 256. */
+SA_API size_t sa_threshold_map_update_workspace_bytes(int B, int H, int NQB, int NKB);
+SA_API sa_status sa_threshold_map_update(const float* sig, const float* levels, int n_levels, float* tmap,
+                                         int B, int H, int NQB, int NKB, void* workspace,
+                                         size_t workspace_bytes, void* stream);
+
 /* FAST's Fidelity Score from the forward pass's log-sum-exp (Eq. 3 Hellinger distance,
  * PAPER.md:132-134 Eq. 4 F = 1 - H, PAPER.md:155-159 stratified row sample; reading P17):
  * with P the dense softmax row and P~ the softmax over the kept keys only,

@@ -55,6 +55,10 @@ def load_library() -> C.CDLL:
     lib.sa_mask_from_threshold.argtypes = [vp, vp, vp, ip, ip, ip, ip, ip, ip, vp]
     lib.sa_block_significance.restype = ip
     lib.sa_block_significance.argtypes = [vp, vp, vp, vp, ip, ip, ip, ip, ip, ip, ip, fp, vp]
+    lib.sa_threshold_map_update_workspace_bytes.restype = sz
+    lib.sa_threshold_map_update_workspace_bytes.argtypes = [ip, ip, ip, ip]
+    lib.sa_threshold_map_update.restype = ip
+    lib.sa_threshold_map_update.argtypes = [vp, vp, ip, vp, ip, ip, ip, ip, vp, sz, vp]
     lib.sa_fidelity_from_lse.restype = ip
     lib.sa_fidelity_from_lse.argtypes = [vp, vp, vp, ip, ip, ip, ip, vp, vp, vp]
     lib.sa_block_sparse_attn_fwd.restype = ip
@@ -192,6 +196,22 @@ def sa_block_significance(q, k, lse, Bq: int, Bk: int, scale: float, n_valid=Non
     _check(lib.sa_block_significance(_ptr(q), _ptr(k), _ptr(lse), _ptr(sig), B, H, N, n_valid, D, Bq,
                                      Bk, float(scale), _stream(stream)))
     return sig
+
+
+def sa_threshold_map_update(sig, levels, tmap, workspace=None, stream=None):
+    """sig fp32 [B][H][NQB][NKB], levels fp32 [n_levels] ascending in (0,1], tmap fp32 [H][NQB][NKB]
+    (in/out, device): tmap <- min(tmap, local map of every sample) (Alg. 1 l.12-17)."""
+    lib = load_library()
+    assert sig.dtype == torch.float32 and sig.is_contiguous() and sig.dim() == 4
+    assert levels.dtype == torch.float32 and levels.is_contiguous() and levels.dim() == 1
+    B, H, NQB, NKB = sig.shape
+    assert tmap.dtype == torch.float32 and tmap.is_contiguous() and tuple(tmap.shape) == (H, NQB, NKB)
+    need = lib.sa_threshold_map_update_workspace_bytes(B, H, NQB, NKB)
+    if workspace is None:
+        workspace = torch.empty(max(need, 256), dtype=torch.uint8, device=sig.device)
+    _check(lib.sa_threshold_map_update(_ptr(sig), _ptr(levels), levels.numel(), _ptr(tmap), B, H, NQB,
+                                       NKB, _ptr(workspace), workspace.numel(), _stream(stream)))
+    return tmap
 
 
 def sa_fidelity_from_lse(lse_dense, lse_sparse, rows, per_row: bool = False, stream=None):

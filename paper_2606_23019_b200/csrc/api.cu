@@ -191,6 +191,34 @@ sa_status sa_block_significance(const void* q, const void* k, const float* lse, 
   return SA_OK;
 }
 
+size_t sa_threshold_map_update_workspace_bytes(int B, int H, int NQB, int NKB) {
+  if (B <= 0 || H <= 0 || NQB <= 0 || NKB <= 0) return 0;
+  if (static_cast<long long>(B) * H * NQB * NKB > 0x7FFFFFFFLL) return 0;
+  return sa::threshold_update_workspace_bytes(B, H, NQB, NKB);
+}
+
+sa_status sa_threshold_map_update(const float* sig, const float* levels, int n_levels, float* tmap, int B,
+                                  int H, int NQB, int NKB, void* workspace, size_t workspace_bytes,
+                                  void* stream) {
+  g_last_launches = 0;
+  if (!sig || !levels || !tmap) return fail(SA_ERR_INVALID_ARG, "sa_threshold_map_update: null pointer");
+  if (B <= 0 || H <= 0 || NQB <= 0 || NKB <= 0 || n_levels <= 0)
+    return fail(SA_ERR_INVALID_ARG, "sa_threshold_map_update: sizes must be positive");
+  if (n_levels > sa::kMaxThresholdLevels || static_cast<long long>(B) * H * NQB * NKB > 0x7FFFFFFFLL)
+    return fail(SA_ERR_UNSUPPORTED, "sa_threshold_map_update: n_levels > %d or B*H*NQB*NKB >= 2^31",
+                sa::kMaxThresholdLevels);
+  const size_t need = sa::threshold_update_workspace_bytes(B, H, NQB, NKB);
+  if (!workspace || workspace_bytes < need || (reinterpret_cast<uintptr_t>(workspace) & 255u))
+    return fail(SA_ERR_WORKSPACE, "sa_threshold_map_update: workspace %zu B < %zu B or not 256 B aligned",
+                workspace_bytes, need);
+  sa_status s = check_device();
+  if (s != SA_OK) return s;
+  cudaError_t e = sa::launch_threshold_update(sig, levels, n_levels, tmap, B, H, NQB, NKB, workspace,
+                                              static_cast<cudaStream_t>(stream), &g_last_launches);
+  if (e != cudaSuccess) return cuda_fail(e, "sa_threshold_map_update launch");
+  return SA_OK;
+}
+
 sa_status sa_fidelity_from_lse(const float* lse_dense, const float* lse_sparse, const int32_t* rows,
                                int n_rows, int B, int H, int N, float* fidelity, float* per_row,
                                void* stream) {

@@ -97,6 +97,11 @@ bool make_tile_map_128x64(void* map /* CUtensorMap* */, const void* base, uint64
 cudaError_t launch_block_significance(const __nv_bfloat16* q, const __nv_bfloat16* k, const float* lse,
                                       float* sig, int B, int H, int N, int n_valid, float scale,
                                       cudaStream_t st, const char** err_text);
+size_t threshold_update_workspace_bytes(int B, int H, int NQB, int NKB);
+constexpr int kMaxThresholdLevels = 256;
+cudaError_t launch_threshold_update(const float* sig, const float* levels, int n_levels, float* tmap,
+                                    int B, int H, int NQB, int NKB, void* ws, cudaStream_t st,
+                                    int* n_launch);
 cudaError_t launch_fidelity(const float* lse_dense, const float* lse_sparse, const int32_t* rows,
                             int n_rows, int BH, int N, float* fidelity, float* per_row,
                             cudaStream_t st);

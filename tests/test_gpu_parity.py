@@ -496,6 +496,64 @@ def test_block_significance_matches_eq1(sa):
             assert np.abs(sig[b, h].sum(axis=1) - rows / (blk * blk)).max() < 1e-6   # row mass
 
 
+@pytest.mark.parametrize("B,H,NQB,NKB", [(1, 2, 4, 4), (3, 2, 7, 5), (2, 3, 40, 40), (1, 1, 1, 1),
+                                         (2, 2, 91, 91)])
+def test_threshold_map_update_matches_alg1(sa, B, H, NQB, NKB):
+    # Alg. 1 l.12-17 on synthetic heavy-tailed significances with ties; the map must come out
+    # level for level as the oracle's (the cumulative sums differ in association order only: a level
+    # could flip only if C/total fell within ~1e-15 of it, which the discrete check would expose).
+    rng = np.random.Generator(np.random.PCG64(B * 1000 + NQB))
+    sig = (rng.random((B, H, NQB, NKB)) ** 6).astype(np.float32)
+    if NQB > 1:
+        sig[:, :, 0, 0] = sig[:, :, 1, 1]                      # ties
+        sig[0, 0, -1, -1] = 0.0                                # a zero block
+    levels = (np.arange(1, 49) / 48.0).astype(np.float32)      # 48 levels, last = 1.0
+    T0 = np.ones((H, NQB, NKB), dtype=np.float32)
+    T0[0, 0, 0] = levels[5]                                     # an earlier sample already set this one
+    ref = T0.astype(np.float64)
+    for b in range(B):
+        for h in range(H):
+            ref[h] = oracle_west.threshold_map_update(ref[h], sig[b, h], levels)
+    tmap = torch.from_numpy(T0.copy()).cuda()
+    sa.sa_threshold_map_update(torch.from_numpy(sig).cuda(), torch.from_numpy(levels).cuda(), tmap)
+    torch.cuda.synchronize()
+    got = tmap.cpu().numpy()
+    assert np.array_equal(got.astype(np.float64), ref), np.abs(got - ref).max()
+
+
+def test_west_pipeline_dense_lse_to_mask(sa):
+    # the paper's offline path end to end on synthetic q, k (no calibration prompts here): dense
+    # forward -> lse -> Eq. 1 -> Alg. 1 l.12-17 -> M_p = 1(T <= p) -> sparse forward -> fidelity
+    D, blk, H, nblk = 128, 128, 2, 8
+    N = nblk * blk
+    g = torch.Generator().manual_seed(41)
+    q = (torch.randn((2, H, N, D), generator=g) * 2).to(torch.bfloat16).cuda()
+    k = torch.randn((2, H, N, D), generator=g).to(torch.bfloat16).cuda()
+    v = torch.randn((2, H, N, D), generator=g).to(torch.bfloat16).cuda()
+    scale = float(np.float32(1 / math.sqrt(D)))
+    ones = dev_bits(oracle.pack_bool(np.ones((H, nblk, nblk), dtype=bool)))
+    _, lse_d = sa.sa_block_sparse_attn_fwd_ex(q, k, v, ones, blk, blk, scale)
+    sig = sa.sa_block_significance(q, k, lse_d, blk, blk, scale)
+    levels = torch.from_numpy((np.arange(1, 21) / 20.0).astype(np.float32)).cuda()
+    tmap = torch.ones((H, nblk, nblk), dtype=torch.float32, device="cuda")
+    sa.sa_threshold_map_update(sig, levels, tmap)
+    p_star = torch.tensor([0.6, 0.8], dtype=torch.float32, device="cuda")
+    bits = sa.sa_mask_from_threshold(tmap, p_star, nblk, nblk, force_diag=False)
+    _, lse_s = sa.sa_block_sparse_attn_fwd_ex(q, k, v, bits, blk, blk, scale)
+    rows = torch.arange(0, N, 37, dtype=torch.int32, device="cuda")
+    fid, per_row = sa.sa_fidelity_from_lse(lse_d, lse_s, rows, per_row=True)
+    torch.cuda.synchronize()
+    # the union mask keeps at least the mass fraction p* of EVERY sample's head: rho >= p* on average,
+    # i.e. mean over rows of exp(lse_s - lse_d) >= p* (mass is averaged over rows by Eq. 1)
+    rho = torch.exp(lse_s - lse_d).mean(dim=2).cpu().numpy()
+    assert (rho[:, 0] >= 0.6 - 1e-3).all() and (rho[:, 1] >= 0.8 - 1e-3).all()
+    fid = fid.cpu().numpy()
+    assert ((fid > 0.3) & (fid <= 1.0)).all() and (fid[:, 0] < 1.0).all()
+    dens = oracle.unpack_mask(host_bits(bits), nblk).mean(axis=(1, 2))
+    assert 0 < dens[0] <= dens[1] <= 1.0          # a larger p* keeps a superset (nested masks)
+    assert (fid[:, 0] <= fid[:, 1]).all()
+
+
 def test_host_buffer_entry_point(sa):
     cfg = inputs.C1
     q, k, v = inputs.make_qkv(cfg, pin_memory=True)
