@@ -261,6 +261,60 @@ def run_seq_grid(sa, dev, stream, peaks, H: int, log):
     return rows
 
 
+def run_west_offline(sa, dev, stream, peaks, log):
+    """the per-sample offline steps at Wan2.1-14B 480p shapes (C3:
+    H=40, N=32768, 32760 valid) on synthetic q, k: dense forward (for lse), block significance
+    (Eq. 1), threshold-map update (Alg. 1 l.12-17, 48 levels), fidelity from lse (Eq. 3-4)."""
+    import numpy as np
+    import torch
+    from paper_2606_23019_b200 import inputs
+    cfg = inputs.C3
+    g = torch.Generator(device=dev).manual_seed(cfg.qkv_seed)
+    q, k, v = [torch.randn((cfg.B, cfg.H, cfg.N, cfg.D), generator=g, device=dev,
+                           dtype=torch.float32).to(torch.bfloat16) for _ in range(3)]
+    ones = torch.full((cfg.H, cfg.NQB, cfg.W), -1, dtype=torch.int32, device=dev)
+    out, lse_d = sa.sa_block_sparse_attn_fwd_ex(q, k, v, ones, cfg.Bq, cfg.Bk, cfg.scale, cfg.n_valid)
+    sig = torch.empty((cfg.B, cfg.H, cfg.NQB, cfg.NKB), dtype=torch.float32, device=dev)
+    levels = torch.from_numpy((np.arange(1, 49) / 48.0).astype(np.float32)).to(dev)
+    tmap = torch.ones((cfg.H, cfg.NQB, cfg.NKB), dtype=torch.float32, device=dev)
+    ws = torch.empty(sa.load_library().sa_threshold_map_update_workspace_bytes(cfg.B, cfg.H, cfg.NQB, cfg.NKB),
+                     dtype=torch.uint8, device=dev)
+    rows = torch.arange(7, cfg.n_valid, 2048, dtype=torch.int32, device=dev)     # 16 rows (Sec. 4.2.3)
+
+    def timed(fn, reps):
+        fn()
+        torch.cuda.synchronize()
+        ts = []
+        for _ in range(reps):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            fn()
+            b.record(stream)
+            torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        return statistics.median(ts)
+
+    t_sig = timed(lambda: sa.sa_block_significance(q, k, lse_d, cfg.Bq, cfg.Bk, cfg.scale, cfg.n_valid, sig, stream), 5)
+    t_upd = timed(lambda: sa.sa_threshold_map_update(sig, levels, tmap, ws, stream), 5)
+    t_fid = timed(lambda: sa.sa_fidelity_from_lse(lse_d, lse_d, rows, stream=stream), 10)
+    tiles = cfg.B * cfg.H * cfg.NQB * cfg.NKB
+    exps = tiles * cfg.Bq * cfg.Bk
+    mufu_peak = 16 * 148 * peaks.get("sm_max_mhz", 1965.0) * 1e6          # ex2 per second at max clock
+    res = {"shape": cfg.name,
+           "block_significance": {"ms": t_sig, "tiles": tiles, "bound": "alu",
+                                  "achieved": exps / (t_sig * 1e-3) / 1e12, "peak": mufu_peak / 1e12,
+                                  "unit": "Texp2/s", "frac": exps / (t_sig * 1e-3) / mufu_peak,
+                                  "peak_kind": "16 MUFU.EX2/clk/SM x 148 SMs x max SM clock",
+                                  "qk_tflops": tiles * 2 * cfg.Bq * cfg.Bk * cfg.D / (t_sig * 1e-3) / 1e12},
+           "threshold_map_update": {"ms": t_upd, "blocks": tiles, "levels": 48,
+                                    "mblocks_per_s": tiles / (t_upd * 1e-3) / 1e6},
+           "fidelity_from_lse": {"ms": t_fid, "rows": int(rows.numel())}}
+    log(f"[bench] west offline at {cfg.name}: significance {t_sig:.3f} ms "
+        f"({res['block_significance']['frac']:.2f} of the MUFU peak), map update {t_upd:.3f} ms, "
+        f"fidelity {t_fid:.4f} ms")
+    return res
+
+
 def run_ours(args, rank: int, local_rank: int, world: int) -> int:
     import numpy as np
     import torch
@@ -426,6 +480,10 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> int:
     if rank == 0 and args.seqlen_grid:
         seq_grid = run_seq_grid(sa, dev, stream, peaks, args.grid_heads, log)
 
+    west = None
+    if rank == 0 and args.west:
+        west = run_west_offline(sa, dev, stream, peaks, log)
+
     # ---- pack-mask kernel group on its own (HBM/ALU-bound; not the dominant kernel)
     pack_ms = None
     if rank == 0:
@@ -564,6 +622,7 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> int:
             "cpu_baseline": cpu_baseline,
             "density_sweep": sweep,
             "seqlen_grid": seq_grid,
+            "west_offline": west,
         }
         print(json.dumps(line), flush=True)
     if dist is not None:
@@ -588,6 +647,9 @@ def main() -> int:
                     help="also time the sequence-length x density grid (1K..262K tokens) and a "
                          "HunyuanVideo-shaped layer; off by default to keep the default run short")
     ap.add_argument("--grid-heads", type=int, default=12)
+    ap.add_argument("--west", action="store_true",
+                    help="also time the offline per-sample steps (block significance, threshold-map "
+                         "update, fidelity) at Wan2.1-14B 480p shapes")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
