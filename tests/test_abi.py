@@ -91,6 +91,30 @@ def test_pack_and_misc_validation(lib):
     assert host(None, 16, 16, 16, 16, 16, 1, 2, 1024, 1024, 64, 64, 64, 0.125, 256, 1 << 30, None) == INVALID
 
 
+def test_offline_entry_points_validation(lib):
+    INVALID, UNSUPPORTED, WORKSPACE = 1, 2, 4
+    mft = lib.sa_mask_from_threshold
+    assert mft(None, 16, 16, 2, 4, 4, 8, 8, 1, None) == INVALID
+    assert mft(16, 16, 16, 2, 0, 4, 8, 8, 1, None) == INVALID
+    assert mft(24, 16, 16, 2, 4, 4, 8, 8, 1, None) == INVALID            # misaligned map
+    assert mft(16, 16, 16, 2, 4, 4, 40000, 8, 1, None) == UNSUPPORTED    # grid side > 32768
+    sig = lib.sa_block_significance
+    assert sig(None, 16, 16, 16, 1, 2, 1024, 1024, 128, 128, 128, 0.1, None) == INVALID
+    assert sig(16, 16, 16, 16, 1, 2, 1000, 1000, 128, 128, 128, 0.1, None) == INVALID
+    assert sig(16, 16, 16, 16, 1, 2, 1024, 1024, 64, 64, 64, 0.1, None) == UNSUPPORTED
+    upd = lib.sa_threshold_map_update
+    assert lib.sa_threshold_map_update_workspace_bytes(2, 3, 40, 40) > 2 * 2 * 3 * 1600 * 8
+    assert lib.sa_threshold_map_update_workspace_bytes(0, 3, 40, 40) == 0
+    assert upd(None, 16, 4, 16, 1, 2, 8, 8, 256, 1 << 30, None) == INVALID
+    assert upd(16, 16, 0, 16, 1, 2, 8, 8, 256, 1 << 30, None) == INVALID
+    assert upd(16, 16, 300, 16, 1, 2, 8, 8, 256, 1 << 30, None) == UNSUPPORTED
+    assert upd(16, 16, 4, 16, 1, 2, 8, 8, 256, 8, None) == WORKSPACE
+    assert upd(16, 16, 4, 16, 1, 2, 8, 8, 8, 1 << 30, None) == WORKSPACE   # not 256 B aligned
+    fid = lib.sa_fidelity_from_lse
+    assert fid(None, 16, 16, 4, 1, 2, 1024, 16, None, None) == INVALID
+    assert fid(16, 16, 16, 0, 1, 2, 1024, 16, None, None) == INVALID
+
+
 def test_product_does_not_import_oracle():
     # the product path must not route through the oracle (or any CPU fallback)
     pkg = os.path.join(ROOT, "paper_2606_23019_b200")
