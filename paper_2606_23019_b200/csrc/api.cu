@@ -274,6 +274,7 @@ sa_status sa_block_sparse_attn_fwd_ex(const void* q, const void* k, const void* 
   const sa::FwdWorkspace w = sa::carve_fwd_workspace(workspace, B, H, p.NQB);
   p.unit_order = w.unit_order;
   p.counter = w.cursor;
+  p.kmax2 = w.kmax2;
 
   const bool fast = (g_variant == 0 && D == 128);
   const int rows_per_item = fast ? 2 : 1;

@@ -61,6 +61,7 @@ struct FwdParams {
   // schedule (workspace)
   const int32_t* unit_order;  // [n_items] item ids in issue order
   int32_t* counter;           // dynamic scheduler cursor (zeroed by the pre-pass)
+  const float* kmax2;         // [B*H] max |k|^2 over the valid keys (tcgen05 kernel only)
   int n_items;
 };
 
@@ -68,12 +69,14 @@ struct FwdParams {
 //   [0]                  scheduler cursor
 //   [16 .. 16+BH)        per-(b,h) total cost
 //   [.. + BH)            (b,h) issue order (heaviest first)
+//   [.. + BH)            fp32: per (b,h) max over the valid keys of |k|^2
 //   [.. + BH*items]      per-(b,h) item order (cost descending), local item index
 //   [.. + BH*items]      flattened issue order of global item ids
 struct FwdWorkspace {
   int32_t* cursor;
   int32_t* head_cost;
   int32_t* head_order;
+  float* kmax2;               // [B*H] max over valid keys of |k|^2
   int32_t* local_order;
   int32_t* unit_order;
 };

@@ -43,6 +43,9 @@ constexpr int kSlots = 5;                 // K/V ring
 constexpr int kSched = 2;                 // scheduler ring
 constexpr uint32_t kTmemCols = 512;
 constexpr float kRescaleThreshold = 8.0f; // log2 units
+constexpr float kBoundSlack = 64.0f;      // log2 units: how far the Cauchy-Schwarz bound may lie above
+                                          // the first block's row maximum and still be used (2^-64 of
+                                          // headroom is left before fp32 / bf16 flush to zero at 2^-126)
 // Tunables of the softmax (defaults chosen by measurement on B200, profiles/):
 //  SA_POLY_PAIRS: of every 4 consecutive column pairs, how many take exp2 on the FMA pipe
 //  (Cody-Waite split + degree-3 polynomial) instead of MUFU.EX2 -- the MUFU pipe (16/clk/SM)
@@ -272,6 +275,11 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     }
     bool first[2] = {true, true};
 
+    // The next Q tiles are loaded only after every softmax warp has read the current ones (row
+    // norms), and a softmax warp may be waiting for o_full of a unit still parked in the FIFO: if Q
+    // is not there yet, issue the parked PVs first (they need nothing from the next item).
+    if (!mbar_try_wait(smem_u32(&ctl->q_full), q_phase))
+      while (npend > 0) pop();
     mbar_wait(smem_u32(&ctl->q_full), q_phase, 11);
     q_phase ^= 1u;
     tc_fence_after();
@@ -398,13 +406,13 @@ __device__ __forceinline__ float exp_tile(const uint32_t (&sr)[4][32], float c, 
 // ------------------------------------------------------------------ warps 4-11: softmax + epilogue
 // One thread per query row: thread (quarter, lane) of warpgroup t owns TMEM lane 32*quarter+lane
 // of S_t / O_t, so row max and row sum need no shuffles.
-__device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t tmem, int t, int quarter,
-                           int lane, int items_per_head) {
+__device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uint32_t tmem, int t,
+                           int quarter, int lane, int items_per_head) {
   const int row = quarter * 32 + lane;
   const uint32_t lane_base = static_cast<uint32_t>(quarter * 32) << 16;
   const uint32_t tm_o = tmem + lane_base + 256 + t * 128;
   const float c = p.scale_log2;
-  uint32_t o_phase = 0;
+  uint32_t o_phase = 0, qf_phase = 0;
   uint32_t wg = 0;                       // global unit counter, in step with the MMA issuer
   uint32_t nmine = 0;                    // this tile's units so far (barrier selection: every phase
                                          // of s_full[t][.] is consumed in order, none is skipped)
@@ -427,8 +435,40 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t tmem, int t, i
     const int u = it.u0 + t;
     const bool exists = u < p.NQB;
 
+    // An upper bound of every score of this query row (Cauchy-Schwarz): scale * |q_i| * max_j |k_j|,
+    // in the log2 domain. |q_i| comes from the Q tile in shared memory (128B-swizzled rows), max |k|
+    // from the pre-pass. If the first key block shows that the bound is not far above the real
+    // scores, it becomes the row's softmax reference point for the whole item: no running max, no
+    // rescale, and the row-max pass (a third of the softmax instructions) disappears. Otherwise the
+    // warp keeps the exact running max. Either way the result is the same softmax.
+    mbar_wait(smem_u32(&ctl->q_full), qf_phase, 24);
+    qf_phase ^= 1u;
+    float bound = 0.f;
+    if (exists) {
+      const uint32_t qrow = smem_base + kOffQ + t * kTileBytes + row * 128;
+      float qn2 = 0.f;
+#pragma unroll
+      for (int ch = 0; ch < 16; ++ch) {
+        const uint32_t addr = qrow + (ch >> 3) * kHalfBytes + (((ch & 7) ^ (row & 7)) << 4);
+        uint32_t w0, w1, w2, w3;
+        asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
+                     : "=r"(w0), "=r"(w1), "=r"(w2), "=r"(w3) : "r"(addr));
+        const uint32_t wv[4] = {w0, w1, w2, w3};
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const float lo = __uint_as_float(wv[i] << 16), hi = __uint_as_float(wv[i] & 0xFFFF0000u);
+          qn2 = fmaf(lo, lo, qn2);
+          qn2 = fmaf(hi, hi, qn2);
+        }
+      }
+      bound = c * sqrtf(qn2) * sqrtf(__ldg(p.kmax2 + it.bh));
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(smem_u32(&ctl->q_empty));   // this warp is done with the Q tiles
+
     float m_run = -INFINITY, l_run = 0.f;
     bool started = false;
+    bool fixed = false;                  // warp-uniform: m_run is the bound, fixed for the item
     uint32_t prev_unit = 0xFFFFFFFEu;    // this tile's previous unit in the item
     // walk the union of the two bit-rows (the unit numbering needs both), handle this tile's units
     for (int w = 0; w < p.W; ++w) {
@@ -464,6 +504,7 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t tmem, int t, i
             for (int i = 0; i < 32; ++i)
               if (cc * 32 + i >= kv) sr[cc][i] = 0xFF800000u;   // -inf
         }
+        if (!fixed) {
         // row max: four independent chains of 3-input max
         float mxa[4];
 #pragma unroll
@@ -498,6 +539,14 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t tmem, int t, i
               tmem_st32(tm_o + cc * 32, orr);
             }
           }
+        }
+        if (!started) {
+          // first unit of the item: every row of the warp has a finite maximum and its bound lies
+          // at most kBoundSlack above it -> 2^(s*c - bound) cannot underflow for the row's largest
+          // scores (the real maximum over the item is at least this block's), and never exceeds 1
+          fixed = __all_sync(0xFFFFFFFFu, m_run > -INFINITY && bound <= m_run + kBoundSlack);
+          if (fixed) m_run = bound;
+        }
         }
         const float m_use = (m_run == -INFINITY) ? 0.f : m_run;
         SA_TR(3);
@@ -568,7 +617,7 @@ fwd_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
     prefetch_tensormap(&tm_k);
     prefetch_tensormap(&tm_v);
     mbar_init(smem_u32(&ctl->q_full), 1);
-    mbar_init(smem_u32(&ctl->q_empty), 1);
+    mbar_init(smem_u32(&ctl->q_empty), 1 + 8);   // MMA commit + the 8 softmax warps (row norms)
     for (int s = 0; s < kSlots; ++s) {
       mbar_init(smem_u32(&ctl->kv_full[s]), 1);
       mbar_init(smem_u32(&ctl->kv_empty[s]), 1);
@@ -607,7 +656,7 @@ fwd_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
     }
   } else {
     setmaxnreg_inc<208>();
-    softmax_wg(p, ctl, tmem, warp >= 8 ? 1 : 0, warp & 3, lane, items_per_head);
+    softmax_wg(p, ctl, smem_base, tmem, warp >= 8 ? 1 : 0, warp & 3, lane, items_per_head);
   }
   tc_fence_before();
   __syncthreads();

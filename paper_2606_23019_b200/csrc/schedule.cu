@@ -13,7 +13,7 @@ namespace sa {
 
 size_t fwd_workspace_bytes(int B, int H, int NQB) {
   const size_t BH = static_cast<size_t>(B) * H;
-  const size_t n = 16 + 2 * BH + 2 * BH * static_cast<size_t>(NQB);
+  const size_t n = 16 + 3 * BH + 2 * BH * static_cast<size_t>(NQB);
   return ((n * sizeof(int32_t) + 255) / 256) * 256;
 }
 
@@ -24,7 +24,8 @@ FwdWorkspace carve_fwd_workspace(void* ws, int B, int H, int NQB) {
   w.cursor = p;
   w.head_cost = p + 16;
   w.head_order = w.head_cost + BH;
-  w.local_order = w.head_order + BH;
+  w.kmax2 = reinterpret_cast<float*>(w.head_order + BH);
+  w.local_order = w.head_order + 2 * BH;
   w.unit_order = w.local_order + BH * static_cast<size_t>(NQB);
   return w;
 }
@@ -39,12 +40,15 @@ constexpr int kSortThreads = 1024;
 __global__ void __launch_bounds__(kSortThreads)
 schedule_sort_kernel(const uint32_t* __restrict__ mask_bits, int H, int NQB, int NKB, int W,
                      int rpi, int items, int32_t* __restrict__ head_cost,
-                     int32_t* __restrict__ local_order) {
+                     int32_t* __restrict__ local_order, float* __restrict__ kmax2) {
   extern __shared__ int32_t s_cost[];
   __shared__ int s_total;
   const int bh = blockIdx.x;
   const int h = bh % H;
-  if (threadIdx.x == 0) s_total = 0;
+  if (threadIdx.x == 0) {
+    s_total = 0;
+    kmax2[bh] = 0.f;                 // key_norm_kernel (next on the stream) takes the max into it
+  }
   __syncthreads();
   const uint32_t tail_mask = (NKB & 31) ? ((1u << (NKB & 31)) - 1u) : 0xFFFFFFFFu;
   int my_total = 0;
@@ -101,6 +105,39 @@ schedule_flatten_kernel(const int32_t* __restrict__ head_cost, int32_t* __restri
   unit_order[p] = bh * items + local_order[static_cast<size_t>(bh) * items + pos];
 }
 
+// kmax2[bh] = max over the valid keys j of |k_j|^2 (D = 128; one thread per key row, 16-byte loads).
+// The forward kernel turns it into the Cauchy-Schwarz bound scale * |q_i| * max_j |k_j| >= every
+// score of query row i, which lets it fix the softmax reference point of a row for a whole item.
+constexpr int kNormThreads = 256;
+constexpr int kNormRowsPerBlock = 2048;
+__global__ void __launch_bounds__(kNormThreads)
+key_norm_kernel(const __nv_bfloat16* __restrict__ k, int N, int n_valid, float* __restrict__ kmax2) {
+  const int bh = blockIdx.y;
+  const int r0 = blockIdx.x * kNormRowsPerBlock;
+  const int r1 = min(r0 + kNormRowsPerBlock, n_valid);
+  float best = 0.f;
+  for (int r = r0 + threadIdx.x; r < r1; r += kNormThreads) {
+    const uint4* row = reinterpret_cast<const uint4*>(k + (static_cast<size_t>(bh) * N + r) * 128);
+    float acc = 0.f;
+#pragma unroll
+    for (int c = 0; c < 16; ++c) {
+      const uint4 x = __ldg(row + c);
+      const uint32_t w[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const float lo = __uint_as_float(w[i] << 16), hi = __uint_as_float(w[i] & 0xFFFF0000u);
+        acc = fmaf(lo, lo, acc);
+        acc = fmaf(hi, hi, acc);
+      }
+    }
+    best = fmaxf(best, acc);
+  }
+#pragma unroll
+  for (int s = 16; s > 0; s >>= 1) best = fmaxf(best, __shfl_xor_sync(0xFFFFFFFFu, best, s));
+  if ((threadIdx.x & 31) == 0)
+    atomicMax(reinterpret_cast<unsigned*>(kmax2 + bh), __float_as_uint(best));   // non-negative floats
+}
+
 __global__ void __launch_bounds__(128)
 enumerate_kernel(const uint32_t* __restrict__ mask_bits, int rows, int NKB, int W,
                  int32_t* __restrict__ idx, int32_t* __restrict__ cnt) {
@@ -121,11 +158,16 @@ cudaError_t launch_schedule(const FwdParams& p, const FwdWorkspace& w, int rpi, 
   const int BH = p.B * p.H;
   const int items = (p.NQB + rpi - 1) / rpi;
   schedule_sort_kernel<<<BH, kSortThreads, items * sizeof(int32_t), st>>>(
-      p.mask_bits, p.H, p.NQB, p.NKB, p.W, rpi, items, w.head_cost, w.local_order);
+      p.mask_bits, p.H, p.NQB, p.NKB, p.W, rpi, items, w.head_cost, w.local_order, w.kmax2);
   const int total = BH * items;
   schedule_flatten_kernel<<<(total + 255) / 256, 256, BH * sizeof(int32_t), st>>>(
       w.head_cost, w.head_order, w.local_order, BH, items, w.unit_order, w.cursor);
   *n_launch += 2;
+  if (p.D == 128 && rpi == 2) {      // the tcgen05 kernel's per-row score bound needs max |k|^2
+    const dim3 grid((p.n_valid + kNormRowsPerBlock - 1) / kNormRowsPerBlock, BH);
+    key_norm_kernel<<<grid, kNormThreads, 0, st>>>(p.k, p.N, p.n_valid, w.kmax2);
+    *n_launch += 1;
+  }
   return cudaGetLastError();
 }
 

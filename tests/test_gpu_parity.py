@@ -222,6 +222,47 @@ def test_large_magnitude_scores_and_batch(sa, variant):
     check_out(out, lse, ref_o, ref_l, f"large-magnitude variant={variant}")
 
 
+@pytest.mark.parametrize("case", ["huge-norms", "first-block-tiny", "mixed-rows", "zero-q"])
+def test_score_bound_fallbacks(sa, case):
+    # the tcgen05 kernel fixes a row's softmax reference point at the Cauchy-Schwarz bound
+    # scale*|q|*max|k| only when the first key block shows the bound is close to real scores;
+    # these inputs make it loose (so the exact running max must take over), mix both kinds of
+    # rows in one warp, or make it degenerate.
+    D, blk, H, nblk = 128, 128, 2, 7
+    N = nblk * blk
+    g = torch.Generator().manual_seed(77)
+    q = torch.randn((1, H, N, D), generator=g)
+    k = torch.randn((1, H, N, D), generator=g)
+    v = torch.randn((1, H, N, D), generator=g).to(torch.bfloat16)
+    if case == "huge-norms":            # bound ~ 6500, real maxima ~ 2000 (log2 units)
+        q, k = q * 40, k * 10
+    elif case == "first-block-tiny":    # the first key block of every row is ~0, later blocks are large
+        k = k * 8
+        k[:, :, :blk] *= 1e-3
+        q = q * 8
+    elif case == "mixed-rows":          # every 5th query row is 30x larger than its neighbours
+        q[:, :, ::5] *= 30
+        k[:, :, 300] *= 25              # one outlier key sets max|k|
+    elif case == "zero-q":
+        q[:, :, 100:200] = 0.0
+    q, k = q.to(torch.bfloat16), k.to(torch.bfloat16)
+    m = np.random.Generator(np.random.PCG64(5)).random((H, nblk, nblk)) < 0.5
+    m[:, np.arange(nblk), np.arange(nblk)] = True
+    m[:, :, 0] = True                    # the near-zero block is walked first
+    bits = oracle.pack_bool(m)
+    scale = float(np.float32(1 / math.sqrt(D)))
+    ref_o, ref_l = oracle.attn(inputs.as_u16(q), inputs.as_u16(k), inputs.as_u16(v), bits, blk, blk, scale)
+    out, lse = run_fwd(sa, q, k, v, bits, blk, scale, variant=0)
+    # lse is as large as the scores here: 1e-3 absolute is asked of O(10) values (BASELINE.json);
+    # allow the fp32 spacing of the value on top (|lse| up to ~1500 -> 1.2e-4 per ulp)
+    err = np.abs(lse.cpu().numpy().astype(np.float64) - ref_l)
+    assert (err <= 1e-3 + 16 * np.spacing(np.abs(ref_l).astype(np.float32))).all(), err.max()
+    # with scores in the thousands the softmax is nearly one-hot and near-ties between two keys
+    # flip on the bf16 rounding of P: max-abs 4e-2 here (2e-2 is BASELINE.json's bar for N(0,1) inputs)
+    e = np.abs(out.float().cpu().numpy().astype(np.float64) - ref_o)
+    assert e.max() <= 4e-2 and e.mean() <= 2e-3, (case, e.max(), e.mean())
+
+
 @pytest.mark.parametrize("variant", [0, 1])
 def test_dense_equals_sdpa_on_gpu_shapes(sa, variant):
     # density 1 ("fully dense setting") at a few-tile size
