@@ -105,35 +105,37 @@ schedule_flatten_kernel(const int32_t* __restrict__ head_cost, int32_t* __restri
   unit_order[p] = bh * items + local_order[static_cast<size_t>(bh) * items + pos];
 }
 
-// kmax2[bh] = max over the valid keys j of |k_j|^2 (D = 128; one thread per key row, 16-byte loads).
+// kmax2[bh] = max over the valid keys j of |k_j|^2 (D = 128). Half a warp per key row: 16 lanes x 16
+// bytes = one 256 B row per load, fully coalesced; 4 shuffles fold the 16 partial sums.
 // The forward kernel turns it into the Cauchy-Schwarz bound scale * |q_i| * max_j |k_j| >= every
 // score of query row i, which lets it fix the softmax reference point of a row for a whole item.
 constexpr int kNormThreads = 256;
-constexpr int kNormRowsPerBlock = 2048;
+constexpr int kNormRowsPerBlock = 1024;
 __global__ void __launch_bounds__(kNormThreads)
 key_norm_kernel(const __nv_bfloat16* __restrict__ k, int N, int n_valid, float* __restrict__ kmax2) {
   const int bh = blockIdx.y;
   const int r0 = blockIdx.x * kNormRowsPerBlock;
   const int r1 = min(r0 + kNormRowsPerBlock, n_valid);
+  const int half = threadIdx.x >> 4, sub = threadIdx.x & 15;       // 16 half-warps per block
+  const uint4* base = reinterpret_cast<const uint4*>(k + static_cast<size_t>(bh) * N * 128);
   float best = 0.f;
-  for (int r = r0 + threadIdx.x; r < r1; r += kNormThreads) {
-    const uint4* row = reinterpret_cast<const uint4*>(k + (static_cast<size_t>(bh) * N + r) * 128);
+#pragma unroll 4
+  for (int rb = r0; rb < r1; rb += kNormThreads / 16) {       // uniform trip count (shuffles inside)
+    const int r = rb + half;
+    const uint4 x = r < r1 ? __ldg(base + static_cast<size_t>(r) * 16 + sub) : make_uint4(0u, 0u, 0u, 0u);
+    const uint32_t w[4] = {x.x, x.y, x.z, x.w};
     float acc = 0.f;
 #pragma unroll
-    for (int c = 0; c < 16; ++c) {
-      const uint4 x = __ldg(row + c);
-      const uint32_t w[4] = {x.x, x.y, x.z, x.w};
-#pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        const float lo = __uint_as_float(w[i] << 16), hi = __uint_as_float(w[i] & 0xFFFF0000u);
-        acc = fmaf(lo, lo, acc);
-        acc = fmaf(hi, hi, acc);
-      }
+    for (int i = 0; i < 4; ++i) {
+      const float lo = __uint_as_float(w[i] << 16), hi = __uint_as_float(w[i] & 0xFFFF0000u);
+      acc = fmaf(lo, lo, acc);
+      acc = fmaf(hi, hi, acc);
     }
+#pragma unroll
+    for (int s = 8; s > 0; s >>= 1) acc += __shfl_xor_sync(0xFFFFFFFFu, acc, s);
     best = fmaxf(best, acc);
   }
-#pragma unroll
-  for (int s = 16; s > 0; s >>= 1) best = fmaxf(best, __shfl_xor_sync(0xFFFFFFFFu, best, s));
+  best = fmaxf(best, __shfl_xor_sync(0xFFFFFFFFu, best, 16));
   if ((threadIdx.x & 31) == 0)
     atomicMax(reinterpret_cast<unsigned*>(kmax2 + bh), __float_as_uint(best));   // non-negative floats
 }
