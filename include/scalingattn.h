@@ -161,7 +161,10 @@ SA_API sa_status sa_block_sparse_attn_fwd_ex(const void* q, const void* k, const
 
 /* End-to-end form with HOST buffers (pinned memory recommended): copies q, k, v and the mask to
  * `scratch` (device, >= sa_fwd_host_scratch_bytes, 256 B aligned), runs the forward pass there and
- * copies out and lse back, all on `stream`, without synchronising. */
+ * copies out and lse back, without synchronising. The work is ordered like work queued on `stream`
+ * (it starts after what `stream` holds and `stream` waits for its end), but the uploads and downloads
+ * run on two internal copy streams, pipelined over groups of heads, so that PCIe traffic in both
+ * directions overlaps the forward pass. */
 SA_API sa_status sa_block_sparse_attn_fwd_host(const void* q_host, const void* k_host, const void* v_host,
                                         const uint32_t* mask_bits_host, void* out_host,
                                         float* lse_host, int B, int H, int N, int n_valid, int D,
@@ -171,7 +174,8 @@ SA_API sa_status sa_block_sparse_attn_fwd_host(const void* q_host, const void* k
 /* One pass of the whole hot path with HOST buffers (pinned memory recommended), all on `stream`,
  * without synchronising: copies scores [H][NQB][NKB] and density [H] to the device and packs the
  * mask (sa_pack_mask, force_diag as there), copies q, k, v, runs the forward pass, and copies out,
- * lse and the packed mask (mask_bits_host, uint32 [H][NQB][W], out) back. `scratch` is device
+ * lse and the packed mask (mask_bits_host, uint32 [H][NQB][W], out) back; q, k, v / out, lse are
+ * pipelined over head groups on internal copy streams as in sa_block_sparse_attn_fwd_host. `scratch` is device
  * memory of at least sa_hot_path_host_scratch_bytes(...) bytes, 256 B aligned. */
 SA_API size_t sa_hot_path_host_scratch_bytes(int B, int H, int N, int D, int Bq, int Bk);
 SA_API sa_status sa_hot_path_host(const float* scores_host, const float* density_host, int force_diag,

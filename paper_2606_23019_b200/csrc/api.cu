@@ -92,6 +92,28 @@ struct WsFree {
   }
 } g_ws_free;
 
+// Copy engines for the host-buffer entry points: the q/k/v upload of head group g+1 and the out/lse
+// download of group g-1 overlap the forward pass of group g (PCIe is full duplex and the copy engines
+// run beside the SMs). Two non-blocking streams and a pool of events, created on first use.
+struct PipeCtx {
+  cudaStream_t h2d = nullptr, d2h = nullptr;
+  std::vector<cudaEvent_t> ev;
+  cudaError_t init(size_t n_events) {
+    cudaError_t e = cudaSuccess;
+    if (!h2d && (e = cudaStreamCreateWithFlags(&h2d, cudaStreamNonBlocking)) != cudaSuccess) return e;
+    if (!d2h && (e = cudaStreamCreateWithFlags(&d2h, cudaStreamNonBlocking)) != cudaSuccess) return e;
+    while (ev.size() < n_events) {
+      cudaEvent_t x;
+      if ((e = cudaEventCreateWithFlags(&x, cudaEventDisableTiming)) != cudaSuccess) return e;
+      ev.push_back(x);
+    }
+    return e;
+  }
+};
+std::mutex g_pipe_mu;
+PipeCtx g_pipe;
+constexpr int kPipeGroups = 8;     // head groups per batch entry (fewer when H is small)
+
 }  // namespace
 
 extern "C" {
@@ -239,17 +261,20 @@ sa_status sa_fidelity_from_lse(const float* lse_dense, const float* lse_sparse, 
   return SA_OK;
 }
 
-sa_status sa_block_sparse_attn_fwd_ex(const void* q, const void* k, const void* v,
-                                      const uint32_t* mask_bits, void* out, float* lse, int B,
-                                      int H, int N, int n_valid, int D, int Bq, int Bk,
-                                      float scale, void* workspace, size_t workspace_bytes,
-                                      void* stream) {
+// mask_word_aligned: the pipelined host entry points pass the mask of a head GROUP, which starts at a
+// word boundary inside the caller's 16-byte aligned mask (the kernels read the mask word by word).
+static sa_status fwd_ex_impl(const void* q, const void* k, const void* v, const uint32_t* mask_bits,
+                             void* out, float* lse, int B, int H, int N, int n_valid, int D, int Bq,
+                             int Bk, float scale, void* workspace, size_t workspace_bytes, void* stream,
+                             bool mask_word_aligned) {
   g_last_launches = 0;
   if (!q || !k || !v || !mask_bits || !out || !lse)
     return fail(SA_ERR_INVALID_ARG, "sa_block_sparse_attn_fwd: null pointer");
   sa_status s = validate_shape(B, H, N, n_valid, D, Bq, Bk, scale);
   if (s != SA_OK) return s;
-  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out) || !aligned16(mask_bits) ||
+  const bool mask_ok = mask_word_aligned ? (reinterpret_cast<uintptr_t>(mask_bits) & 3u) == 0
+                                        : aligned16(mask_bits);
+  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out) || !mask_ok ||
       !aligned16(lse) || !aligned16(workspace))
     return fail(SA_ERR_INVALID_ARG, "sa_block_sparse_attn_fwd: pointers must be 16-byte aligned");
   const size_t need = sa::fwd_workspace_bytes(B, H, N / Bq);
@@ -306,6 +331,15 @@ sa_status sa_block_sparse_attn_fwd_ex(const void* q, const void* k, const void* 
   return SA_OK;
 }
 
+sa_status sa_block_sparse_attn_fwd_ex(const void* q, const void* k, const void* v,
+                                      const uint32_t* mask_bits, void* out, float* lse, int B,
+                                      int H, int N, int n_valid, int D, int Bq, int Bk,
+                                      float scale, void* workspace, size_t workspace_bytes,
+                                      void* stream) {
+  return fwd_ex_impl(q, k, v, mask_bits, out, lse, B, H, N, n_valid, D, Bq, Bk, scale, workspace,
+                     workspace_bytes, stream, false);
+}
+
 sa_status sa_block_sparse_attn_fwd(const void* q, const void* k, const void* v,
                                    const uint32_t* mask_bits, void* out, float* lse, int B, int H,
                                    int N, int D, int Bq, int Bk, float scale, void* stream) {
@@ -331,6 +365,62 @@ sa_status sa_block_sparse_attn_fwd(const void* q, const void* k, const void* v,
                                      ws, need, stream);
 }
 
+// q, k, v up / forward / out, lse down, pipelined over head groups (see PipeCtx). The mask is already
+// on the device. Everything is ordered after the work queued on `st` so far, and `st` waits for the
+// last download, so callers see plain stream semantics.
+static sa_status pipelined_fwd_host(const void* q_host, const void* k_host, const void* v_host,
+                                    void* out_host, float* lse_host, char* dq, char* dk, char* dv,
+                                    char* dout, char* dlse, const char* dmask, char* dws, int B, int H,
+                                    int N, int n_valid, int D, int Bq, int Bk, float scale,
+                                    cudaStream_t st, int* launches) {
+  const int groups = H < kPipeGroups ? H : kPipeGroups;
+  const int n_chunks = B * groups;
+  std::lock_guard<std::mutex> lk(g_pipe_mu);
+  cudaError_t e = g_pipe.init(2 * static_cast<size_t>(n_chunks) + 2);
+  if (e != cudaSuccess) return cuda_fail(e, "copy pipeline setup");
+  cudaEvent_t ev_start = g_pipe.ev[0], ev_end = g_pipe.ev[1];
+  if ((e = cudaEventRecord(ev_start, st)) != cudaSuccess ||
+      (e = cudaStreamWaitEvent(g_pipe.h2d, ev_start, 0)) != cudaSuccess ||
+      (e = cudaStreamWaitEvent(g_pipe.d2h, ev_start, 0)) != cudaSuccess)
+    return cuda_fail(e, "copy pipeline fork");
+  const size_t row_bytes = static_cast<size_t>(N) * D * 2;
+  const size_t mask_head_bytes = static_cast<size_t>(N / Bq) * ((N / Bk + 31) / 32) * 4;
+  const size_t ws_bytes = sa_fwd_workspace_bytes(B, H, N, Bq);
+  int c = 0;
+  for (int b = 0; b < B; ++b) {
+    for (int g = 0; g < groups; ++g, ++c) {
+      const int h0 = static_cast<int>(static_cast<long long>(H) * g / groups);
+      const int h1 = static_cast<int>(static_cast<long long>(H) * (g + 1) / groups);
+      const size_t off = (static_cast<size_t>(b) * H + h0) * row_bytes;
+      const size_t bytes = static_cast<size_t>(h1 - h0) * row_bytes;
+      const size_t loff = (static_cast<size_t>(b) * H + h0) * N * 4, lbytes = static_cast<size_t>(h1 - h0) * N * 4;
+      cudaEvent_t ev_in = g_pipe.ev[2 + 2 * c], ev_done = g_pipe.ev[3 + 2 * c];
+      if ((e = cudaMemcpyAsync(dq + off, static_cast<const char*>(q_host) + off, bytes, cudaMemcpyHostToDevice, g_pipe.h2d)) != cudaSuccess ||
+          (e = cudaMemcpyAsync(dk + off, static_cast<const char*>(k_host) + off, bytes, cudaMemcpyHostToDevice, g_pipe.h2d)) != cudaSuccess ||
+          (e = cudaMemcpyAsync(dv + off, static_cast<const char*>(v_host) + off, bytes, cudaMemcpyHostToDevice, g_pipe.h2d)) != cudaSuccess ||
+          (e = cudaEventRecord(ev_in, g_pipe.h2d)) != cudaSuccess ||
+          (e = cudaStreamWaitEvent(st, ev_in, 0)) != cudaSuccess)
+        return cuda_fail(e, "host->device copy (q, k, v)");
+      sa_status s = fwd_ex_impl(
+          dq + off, dk + off, dv + off,
+          reinterpret_cast<const uint32_t*>(dmask + static_cast<size_t>(h0) * mask_head_bytes), dout + off,
+          reinterpret_cast<float*>(dlse + loff), 1, h1 - h0, N, n_valid, D, Bq, Bk, scale, dws, ws_bytes,
+          st, true);
+      if (s != SA_OK) return s;
+      *launches += g_last_launches;
+      if ((e = cudaEventRecord(ev_done, st)) != cudaSuccess ||
+          (e = cudaStreamWaitEvent(g_pipe.d2h, ev_done, 0)) != cudaSuccess ||
+          (e = cudaMemcpyAsync(static_cast<char*>(out_host) + off, dout + off, bytes, cudaMemcpyDeviceToHost, g_pipe.d2h)) != cudaSuccess ||
+          (e = cudaMemcpyAsync(reinterpret_cast<char*>(lse_host) + loff, dlse + loff, lbytes, cudaMemcpyDeviceToHost, g_pipe.d2h)) != cudaSuccess)
+        return cuda_fail(e, "device->host copy");
+    }
+  }
+  if ((e = cudaEventRecord(ev_end, g_pipe.d2h)) != cudaSuccess ||
+      (e = cudaStreamWaitEvent(st, ev_end, 0)) != cudaSuccess)
+    return cuda_fail(e, "copy pipeline join");
+  return SA_OK;
+}
+
 sa_status sa_block_sparse_attn_fwd_host(const void* q_host, const void* k_host, const void* v_host,
                                         const uint32_t* mask_bits_host, void* out_host,
                                         float* lse_host, int B, int H, int N, int n_valid, int D,
@@ -354,18 +444,13 @@ sa_status sa_block_sparse_attn_fwd_host(const void* q_host, const void* k_host, 
   char* dmask = dlse + l;
   char* dws = dmask + m;
   cudaError_t e;
-  if ((e = cudaMemcpyAsync(dq, q_host, tb, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
-      (e = cudaMemcpyAsync(dk, k_host, tb, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
-      (e = cudaMemcpyAsync(dv, v_host, tb, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
-      (e = cudaMemcpyAsync(dmask, mask_bits_host, mb, cudaMemcpyHostToDevice, st)) != cudaSuccess)
-    return cuda_fail(e, "host->device copy");
-  s = sa_block_sparse_attn_fwd_ex(dq, dk, dv, reinterpret_cast<const uint32_t*>(dmask), dout,
-                                  reinterpret_cast<float*>(dlse), B, H, N, n_valid, D, Bq, Bk,
-                                  scale, dws, sa_fwd_workspace_bytes(B, H, N, Bq), stream);
+  if ((e = cudaMemcpyAsync(dmask, mask_bits_host, mb, cudaMemcpyHostToDevice, st)) != cudaSuccess)
+    return cuda_fail(e, "host->device copy (mask)");
+  int launches = 0;
+  s = pipelined_fwd_host(q_host, k_host, v_host, out_host, lse_host, dq, dk, dv, dout, dlse, dmask, dws, B,
+                         H, N, n_valid, D, Bq, Bk, scale, st, &launches);
   if (s != SA_OK) return s;
-  if ((e = cudaMemcpyAsync(out_host, dout, tb, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
-      (e = cudaMemcpyAsync(lse_host, dlse, lb, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
-    return cuda_fail(e, "device->host copy");
+  g_last_launches = launches;
   return SA_OK;
 }
 
@@ -415,19 +500,13 @@ sa_status sa_hot_path_host(const float* scores_host, const float* density_host, 
                    reinterpret_cast<uint32_t*>(dmask), H, NQB, NKB, force_diag, dpws, pack_ws,
                    stream);
   if (s != SA_OK) return s;
-  if ((e = cudaMemcpyAsync(dq, q_host, tb, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
-      (e = cudaMemcpyAsync(dk, k_host, tb, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
-      (e = cudaMemcpyAsync(dv, v_host, tb, cudaMemcpyHostToDevice, st)) != cudaSuccess)
-    return cuda_fail(e, "host->device copy (q, k, v)");
-  s = sa_block_sparse_attn_fwd_ex(dq, dk, dv, reinterpret_cast<const uint32_t*>(dmask), dout,
-                                  reinterpret_cast<float*>(dlse), B, H, N, n_valid, D, Bq, Bk,
-                                  scale, dws, fwd_ws, stream);
+  int launches = sa::kPackMaskLaunches;
+  s = pipelined_fwd_host(q_host, k_host, v_host, out_host, lse_host, dq, dk, dv, dout, dlse, dmask, dws, B,
+                         H, N, n_valid, D, Bq, Bk, scale, st, &launches);
   if (s != SA_OK) return s;
-  g_last_launches += sa::kPackMaskLaunches;
-  if ((e = cudaMemcpyAsync(out_host, dout, tb, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
-      (e = cudaMemcpyAsync(lse_host, dlse, lb, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
-      (e = cudaMemcpyAsync(mask_bits_host, dmask, mb, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
-    return cuda_fail(e, "device->host copy");
+  g_last_launches = launches;
+  if ((e = cudaMemcpyAsync(mask_bits_host, dmask, mb, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+    return cuda_fail(e, "device->host copy (mask)");
   return SA_OK;
 }
 

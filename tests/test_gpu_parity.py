@@ -611,6 +611,40 @@ def test_host_buffer_entry_point(sa):
     check_out(out, lse, ref_o, ref_l, "host entry point")
 
 
+def test_host_entry_points_pipelined_head_groups(sa):
+    # the host-buffer forms upload / compute / download per head group on internal copy streams:
+    # B = 2, H = 11 (uneven groups of 1-2 heads), 7 key blocks (a head's mask is 28 bytes, so a group's
+    # mask starts at a word boundary that is not 16-byte aligned), ragged tail; two calls back to back
+    # on the same scratch; both entry points against the oracle.
+    D, blk, B, H, nblk = 128, 128, 2, 11, 7
+    N, n_valid = nblk * blk, nblk * blk - 19
+    g = torch.Generator().manual_seed(51)
+    q, k, v = [torch.randn((B, H, N, D), generator=g).to(torch.bfloat16).pin_memory() for _ in range(3)]
+    rng = np.random.Generator(np.random.PCG64(52))
+    scores = rng.random((H, nblk, nblk)).astype(np.float32)
+    density = rng.uniform(0.3, 0.8, size=H).astype(np.float32)
+    bits_ref = oracle.pack_mask(scores, density, 1)
+    scale = float(np.float32(1 / math.sqrt(D)))
+    ref_o, ref_l = oracle.attn(inputs.as_u16(q), inputs.as_u16(k), inputs.as_u16(v), bits_ref, blk, blk,
+                               scale, n_valid=n_valid)
+    out = torch.empty_like(q).pin_memory()
+    lse = torch.empty((B, H, N), dtype=torch.float32).pin_memory()
+    bits_h = torch.zeros((H, nblk, 1), dtype=torch.int32).pin_memory()
+    scratch = torch.empty(sa.sa_hot_path_host_scratch_bytes(B, H, N, D, blk, blk), dtype=torch.uint8,
+                          device="cuda")
+    for _ in range(2):
+        out.zero_(); lse.zero_()
+        sa.sa_hot_path_host(torch.from_numpy(scores).pin_memory(), torch.from_numpy(density).pin_memory(),
+                            q, k, v, bits_h, out, lse, blk, blk, scale, n_valid, scratch)
+        torch.cuda.synchronize()
+        assert (bits_h.numpy().view(np.uint32) == bits_ref).all()
+        check_out(out, lse, ref_o, ref_l, "sa_hot_path_host")
+    out.zero_(); lse.zero_()
+    sa.sa_block_sparse_attn_fwd_host(q, k, v, bits_h, out, lse, blk, blk, scale, n_valid, scratch)
+    torch.cuda.synchronize()
+    check_out(out, lse, ref_o, ref_l, "sa_block_sparse_attn_fwd_host")
+
+
 def test_cuda_library_is_the_path(sa):
     # the kernels really ran: launch count reported by the library, and the .so is mapped
     cfg = inputs.C1
