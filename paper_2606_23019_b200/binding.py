@@ -66,6 +66,8 @@ def load_library() -> C.CDLL:
     lib.sa_block_sparse_attn_fwd_ex.restype = ip
     lib.sa_block_sparse_attn_fwd_ex.argtypes = [vp, vp, vp, vp, vp, vp, ip, ip, ip, ip, ip, ip, ip,
                                                 fp, vp, sz, vp]
+    lib.sa_block_sparse_attn_fwd_reuse.restype = ip
+    lib.sa_block_sparse_attn_fwd_reuse.argtypes = lib.sa_block_sparse_attn_fwd_ex.argtypes
     lib.sa_block_sparse_attn_fwd_host.restype = ip
     lib.sa_block_sparse_attn_fwd_host.argtypes = [vp, vp, vp, vp, vp, vp, ip, ip, ip, ip, ip, ip,
                                                   ip, fp, vp, sz, vp]
@@ -257,7 +259,10 @@ def sa_block_sparse_attn_fwd(q, k, v, mask_bits, Bq: int, Bk: int, scale: float,
 
 
 def sa_block_sparse_attn_fwd_ex(q, k, v, mask_bits, Bq: int, Bk: int, scale: float,
-                                n_valid=None, out=None, lse=None, workspace=None, stream=None):
+                                n_valid=None, out=None, lse=None, workspace=None, stream=None,
+                                reuse_schedule: bool = False):
+    """reuse_schedule=True calls sa_block_sparse_attn_fwd_reuse: `workspace` must hold the work list
+    of an earlier call with the same mask and shape."""
     lib = load_library()
     B, H, N, D = _fwd_shapes(q, k, v, mask_bits, Bq, Bk)
     n_valid = N if n_valid is None else int(n_valid)
@@ -268,7 +273,8 @@ def sa_block_sparse_attn_fwd_ex(q, k, v, mask_bits, Bq: int, Bk: int, scale: flo
     if workspace is None:
         workspace = torch.empty(max(lib.sa_fwd_workspace_bytes(B, H, N, Bq), 256),
                                 dtype=torch.uint8, device=q.device)
-    _check(lib.sa_block_sparse_attn_fwd_ex(_ptr(q), _ptr(k), _ptr(v), _ptr(mask_bits), _ptr(out),
+    fn = lib.sa_block_sparse_attn_fwd_reuse if reuse_schedule else lib.sa_block_sparse_attn_fwd_ex
+    _check(fn(_ptr(q), _ptr(k), _ptr(v), _ptr(mask_bits), _ptr(out),
                                            _ptr(lse), B, H, N, n_valid, D, Bq, Bk, float(scale),
                                            _ptr(workspace), workspace.numel(), _stream(stream)))
     return out, lse

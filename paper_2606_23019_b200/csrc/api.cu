@@ -266,7 +266,7 @@ sa_status sa_fidelity_from_lse(const float* lse_dense, const float* lse_sparse, 
 static sa_status fwd_ex_impl(const void* q, const void* k, const void* v, const uint32_t* mask_bits,
                              void* out, float* lse, int B, int H, int N, int n_valid, int D, int Bq,
                              int Bk, float scale, void* workspace, size_t workspace_bytes, void* stream,
-                             bool mask_word_aligned) {
+                             bool mask_word_aligned, bool reuse_schedule = false) {
   g_last_launches = 0;
   if (!q || !k || !v || !mask_bits || !out || !lse)
     return fail(SA_ERR_INVALID_ARG, "sa_block_sparse_attn_fwd: null pointer");
@@ -299,12 +299,14 @@ static sa_status fwd_ex_impl(const void* q, const void* k, const void* v, const 
   const sa::FwdWorkspace w = sa::carve_fwd_workspace(workspace, B, H, p.NQB);
   p.unit_order = w.unit_order;
   p.counter = w.cursor;
-  p.kmax2 = w.kmax2;
+  // the per-row score bound saves ~6% of the attention kernel but costs one more (~8 us) launch:
+  // not worth it on problems of a few thousand tiles, which then keep the exact running max
+  p.kmax2 = static_cast<long long>(B) * H * p.NQB * p.NKB >= 16384 ? w.kmax2 : nullptr;
 
   const bool fast = (g_variant == 0 && D == 128);
   const int rows_per_item = fast ? 2 : 1;
   p.n_items = B * H * ((p.NQB + rows_per_item - 1) / rows_per_item);
-  cudaError_t e = sa::launch_schedule(p, w, rows_per_item, st, &g_last_launches);
+  cudaError_t e = sa::launch_schedule(p, w, rows_per_item, st, &g_last_launches, reuse_schedule);
   if (e != cudaSuccess) return cuda_fail(e, "schedule pre-pass launch");
   cudaEvent_t ev_stop = nullptr;
   {
@@ -338,6 +340,15 @@ sa_status sa_block_sparse_attn_fwd_ex(const void* q, const void* k, const void* 
                                       void* stream) {
   return fwd_ex_impl(q, k, v, mask_bits, out, lse, B, H, N, n_valid, D, Bq, Bk, scale, workspace,
                      workspace_bytes, stream, false);
+}
+
+sa_status sa_block_sparse_attn_fwd_reuse(const void* q, const void* k, const void* v,
+                                         const uint32_t* mask_bits, void* out, float* lse, int B,
+                                         int H, int N, int n_valid, int D, int Bq, int Bk,
+                                         float scale, void* workspace, size_t workspace_bytes,
+                                         void* stream) {
+  return fwd_ex_impl(q, k, v, mask_bits, out, lse, B, H, N, n_valid, D, Bq, Bk, scale, workspace,
+                     workspace_bytes, stream, false, true);
 }
 
 sa_status sa_block_sparse_attn_fwd(const void* q, const void* k, const void* v,

@@ -85,7 +85,7 @@ FwdWorkspace carve_fwd_workspace(void* ws, int B, int H, int NQB);
 
 // launchers (each returns the cudaError_t of its launches; *n_launch += kernels enqueued)
 cudaError_t launch_schedule(const FwdParams& p, const FwdWorkspace& w, int rows_per_item,
-                            cudaStream_t st, int* n_launch);
+                            cudaStream_t st, int* n_launch, bool reuse = false);
 cudaError_t launch_fwd_mma_sync(const FwdParams& p, cudaStream_t st, int* n_launch);
 cudaError_t launch_fwd_tcgen05(const FwdParams& p, void* ws_extra, cudaStream_t st, int* n_launch,
                                const char** err_text);

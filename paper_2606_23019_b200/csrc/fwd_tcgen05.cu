@@ -461,7 +461,7 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
           qn2 = fmaf(hi, hi, qn2);
         }
       }
-      bound = c * sqrtf(qn2) * sqrtf(__ldg(p.kmax2 + it.bh));
+      bound = p.kmax2 ? c * sqrtf(qn2) * sqrtf(__ldg(p.kmax2 + it.bh)) : INFINITY;   // no bound: exact max
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(smem_u32(&ctl->q_empty));   // this warp is done with the Q tiles

@@ -156,16 +156,23 @@ enumerate_kernel(const uint32_t* __restrict__ mask_bits, int rows, int NKB, int 
 }  // namespace
 
 cudaError_t launch_schedule(const FwdParams& p, const FwdWorkspace& w, int rpi, cudaStream_t st,
-                            int* n_launch) {
+                            int* n_launch, bool reuse) {
   const int BH = p.B * p.H;
   const int items = (p.NQB + rpi - 1) / rpi;
+  if (reuse) {
+    // the work list in the workspace is still valid (same mask): only reset what a call consumes
+    cudaError_t e = cudaMemsetAsync(w.cursor, 0, sizeof(int32_t), st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(w.kmax2, 0, static_cast<size_t>(BH) * sizeof(float), st);
+    if (e != cudaSuccess) return e;
+  } else {
   schedule_sort_kernel<<<BH, kSortThreads, items * sizeof(int32_t), st>>>(
       p.mask_bits, p.H, p.NQB, p.NKB, p.W, rpi, items, w.head_cost, w.local_order, w.kmax2);
   const int total = BH * items;
   schedule_flatten_kernel<<<(total + 255) / 256, 256, BH * sizeof(int32_t), st>>>(
       w.head_cost, w.head_order, w.local_order, BH, items, w.unit_order, w.cursor);
   *n_launch += 2;
-  if (p.D == 128 && rpi == 2) {      // the tcgen05 kernel's per-row score bound needs max |k|^2
+  }
+  if (p.D == 128 && rpi == 2 && p.kmax2 != nullptr) {   // the tcgen05 kernel's score bound needs max |k|^2
     const dim3 grid((p.n_valid + kNormRowsPerBlock - 1) / kNormRowsPerBlock, BH);
     key_norm_kernel<<<grid, kNormThreads, 0, st>>>(p.k, p.N, p.n_valid, w.kmax2);
     *n_launch += 1;
