@@ -11,19 +11,23 @@
 //     pre-pass with an atomic cursor, so uneven rows and heads balance out.
 //   * the two query tiles have different bit-rows; the CTA walks the UNION of the two rows, stages
 //     each K/V tile of the union ONCE (TMA, 128B swizzle, 5-slot ring of 32 KB tiles), and issues
-//     the MMAs of a tile only where that tile's own bit is set. Adjacent query blocks of a
-//     3D-local mask share most key blocks, so L2->SM traffic per active block nearly halves.
-//   * warp 0: scheduler + TMA producer; warp 1: tcgen05.mma issuer (one thread); warp 2: TMEM
-//     allocator; warps 4-7 / 8-11: softmax warpgroups of query tile 0 / 1 (one thread per row).
-//   * TMEM (512 columns): S0 [0,128) S1 [128,256) O0 [256,384) O1 [384,512), fp32. P (bf16, two
-//     per column) overwrites the first 64 columns of its S and feeds the PV MMA as the TMEM
-//     A operand, so P never touches shared memory.
-//   * MMA issue order S0(j) PV1(j-1) S1(j) PV0(j): the softmax of one tile overlaps the MMAs of
-//     the other.
-//   * online softmax in the log2 domain with the scale folded into one FFMA; the running max is
-//     only raised when it grows by more than 8 (factor 256), which keeps the O accumulator
-//     rescale (a TMEM round trip) off the common path without changing the result beyond fp32
-//     rounding: out and lse use the same (possibly stale) max consistently.
+//     the MMAs of a tile only where that tile's own bit is set, so a key block both rows have is
+//     read from L2 once.
+//   * warp 0: scheduler + TMA producer; warp 1: tcgen05.mma issuer; both run converged and issue
+//     through elect.sync (uniform-register UTCHMMA / UTMALDG); warp 2: TMEM allocator; warps 4-7 /
+//     8-11: softmax warpgroups of query tile 0 / 1 (one thread per row).
+//   * TMEM (512 columns): two S/P buffers [0,128) [128,256), O0 [256,384) O1 [384,512), fp32. P
+//     (bf16, two per column) overwrites the first 64 columns of its S and feeds the PV MMA as the
+//     TMEM A operand, so P never touches shared memory.
+//   * (tile, key block) units are numbered in walk order; unit w uses buffer w & 1 and the issue
+//     order is PV(w-2), S(w): the softmax of one unit overlaps the MMAs of its neighbours whether
+//     the neighbours belong to the other tile or to the same one.
+//   * softmax in the log2 domain, scale folded into one FFMA2. A row's reference point is normally
+//     the Cauchy-Schwarz bound scale*|q_i|*max|k| (>= every score), fixed for the whole item: no
+//     running max, no rescale. If the first key block shows the bound is too loose, the warp keeps
+//     the exact running max, raised only when it grows by more than 8 (factor 256), which keeps the
+//     O rescale (a TMEM round trip) off the common path; out and lse use the same reference point
+//     consistently, so the result is the same softmax either way.
 #include <cuda.h>
 
 #include "common.cuh"
