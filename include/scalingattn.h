@@ -214,9 +214,13 @@ SA_API sa_status sa_enumerate_active_blocks(const uint32_t* mask_bits, int H, in
                                      int32_t* idx, int32_t* cnt, void* stream);
 
 /* Which CUDA kernel the forward pass uses. 0 (default): automatic -- the tcgen05/TMEM/TMA kernel
- * for (128,128,128), the mma.sync kernel for (64,64,64). 1: the mma.sync kernel for every
- * supported shape (a second CUDA implementation kept for cross-checking; not a fallback: it is
- * never chosen implicitly for a shape the fast kernel supports). Process-wide. */
+ * for (128,128,128), the mma.sync kernel for (64,64,64); the tcgen05 kernel takes work items of two
+ * adjacent query blocks (shared K/V tiles) unless the problem has fewer than two waves of such pairs,
+ * in which case it takes single query blocks. 1: the mma.sync kernel for every supported shape (a
+ * second CUDA implementation kept for cross-checking; not a fallback: it is never chosen implicitly
+ * for a shape the fast kernel supports). 2 / 3: the tcgen05 kernel with its large-problem path (pair
+ * items, key-norm pre-pass and score bound) / its small-problem path (single-block items, exact running
+ * max) forced, so that tests can drive either on any size. Process-wide. */
 SA_API sa_status sa_set_fwd_variant(int variant);
 SA_API int sa_get_fwd_variant(void);
 

@@ -299,12 +299,16 @@ static sa_status fwd_ex_impl(const void* q, const void* k, const void* v, const 
   const sa::FwdWorkspace w = sa::carve_fwd_workspace(workspace, B, H, p.NQB);
   p.unit_order = w.unit_order;
   p.counter = w.cursor;
+  const bool fast = (g_variant != 1 && D == 128);
   // the per-row score bound saves ~6% of the attention kernel but costs one more (~8 us) launch:
   // not worth it on problems of a few thousand tiles, which then keep the exact running max
-  p.kmax2 = static_cast<long long>(B) * H * p.NQB * p.NKB >= 16384 ? w.kmax2 : nullptr;
-
-  const bool fast = (g_variant == 0 && D == 128);
-  const int rows_per_item = fast ? 2 : 1;
+  const bool big = static_cast<long long>(B) * H * p.NQB * p.NKB >= 16384;
+  p.kmax2 = (fast && (g_variant == 2 || (g_variant == 0 && big))) ? w.kmax2 : nullptr;
+  // The tcgen05 kernel works on PAIRS of query blocks (shared K/V tiles). When there are fewer pairs
+  // than two waves of CTAs (short sequences) single-row items fill the SMs better.
+  const long long n_pairs = static_cast<long long>(B) * H * ((p.NQB + 1) / 2);
+  const int rows_per_item = (fast && (g_variant == 2 || (g_variant == 0 && n_pairs >= 2 * 148))) ? 2 : 1;
+  p.rows_per_item = rows_per_item;
   p.n_items = B * H * ((p.NQB + rows_per_item - 1) / rows_per_item);
   cudaError_t e = sa::launch_schedule(p, w, rows_per_item, st, &g_last_launches, reuse_schedule);
   if (e != cudaSuccess) return cuda_fail(e, "schedule pre-pass launch");
@@ -567,8 +571,8 @@ sa_status sa_enumerate_active_blocks(const uint32_t* mask_bits, int H, int NQB, 
 }
 
 sa_status sa_set_fwd_variant(int variant) {
-  if (variant != 0 && variant != 1)
-    return fail(SA_ERR_INVALID_ARG, "sa_set_fwd_variant: variant %d not in {0,1}", variant);
+  if (variant < 0 || variant > 3)
+    return fail(SA_ERR_INVALID_ARG, "sa_set_fwd_variant: variant %d not in {0,1,2,3}", variant);
   g_variant = variant;
   return SA_OK;
 }

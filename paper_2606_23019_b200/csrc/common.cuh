@@ -63,6 +63,7 @@ struct FwdParams {
   int32_t* counter;           // dynamic scheduler cursor (zeroed by the pre-pass)
   const float* kmax2;         // [B*H] max |k|^2 over the valid keys (tcgen05 kernel only)
   int n_items;
+  int rows_per_item;          // query blocks per work item: 2 (a pair shares its K/V tiles) or 1
 };
 
 // Workspace layout for the forward pass (all int32):

@@ -110,8 +110,8 @@ __device__ __forceinline__ Item decode_item(const FwdParams& p, int item, int it
   Item it;
   it.bh = item / items_per_head;
   it.h = it.bh % p.H;
-  it.u0 = 2 * (item % items_per_head);
-  it.has1 = it.u0 + 1 < p.NQB;
+  it.u0 = p.rows_per_item * (item % items_per_head);
+  it.has1 = p.rows_per_item == 2 && it.u0 + 1 < p.NQB;   // single-row items leave tile 1 empty
   it.row0 = it.bh * p.N;
   return it;
 }
@@ -437,7 +437,7 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     if (item < 0) break;
     const Item it = decode_item(p, item, items_per_head);
     const int u = it.u0 + t;
-    const bool exists = u < p.NQB;
+    const bool exists = t == 0 || it.has1;   // tile 1 is empty in single-row items and past the last row
 
     // An upper bound of every score of this query row (Cauchy-Schwarz): scale * |q_i| * max_j |k_j|,
     // in the log2 domain. |q_i| comes from the Q tile in shared memory (128B-swizzled rows), max |k|
@@ -614,7 +614,7 @@ fwd_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
   const uint32_t smem_base = (raw + 1023u) & ~1023u;
   Ctl* ctl = reinterpret_cast<Ctl*>(smem_raw + (smem_base - raw) + kOffCtl);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int items_per_head = (p.NQB + 1) / 2;
+  const int items_per_head = (p.NQB + p.rows_per_item - 1) / p.rows_per_item;
 
   if (threadIdx.x == 0) {
     prefetch_tensormap(&tm_q);

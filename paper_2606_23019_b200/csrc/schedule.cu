@@ -172,7 +172,7 @@ cudaError_t launch_schedule(const FwdParams& p, const FwdWorkspace& w, int rpi, 
       w.head_cost, w.head_order, w.local_order, BH, items, w.unit_order, w.cursor);
   *n_launch += 2;
   }
-  if (p.D == 128 && rpi == 2 && p.kmax2 != nullptr) {   // the tcgen05 kernel's score bound needs max |k|^2
+  if (p.D == 128 && p.kmax2 != nullptr) {   // the tcgen05 kernel's score bound needs max |k|^2
     const dim3 grid((p.n_valid + kNormRowsPerBlock - 1) / kNormRowsPerBlock, BH);
     key_norm_kernel<<<grid, kNormThreads, 0, st>>>(p.k, p.N, p.n_valid, w.kmax2);
     *n_launch += 1;

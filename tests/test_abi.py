@@ -83,7 +83,8 @@ def test_pack_and_misc_validation(lib):
     assert lib.sa_pack_mask(16, 16, 16, 2, 16, 16, 1, 16, 8, None) == WORKSPACE
     assert lib.sa_pack_mask(16, 16, 16, 2, 16, 16, 1, None, 1 << 20, None) == WORKSPACE
     assert lib.sa_enumerate_active_blocks(None, 1, 1, 1, 16, 16, None) == INVALID
-    assert lib.sa_set_fwd_variant(7) == INVALID
+    assert lib.sa_set_fwd_variant(7) == INVALID and lib.sa_set_fwd_variant(-1) == INVALID
+    assert lib.sa_set_fwd_variant(3) == 0 and lib.sa_set_fwd_variant(2) == 0
     assert lib.sa_set_fwd_variant(1) == 0 and lib.sa_get_fwd_variant() == 1
     assert lib.sa_set_fwd_variant(0) == 0 and lib.sa_get_fwd_variant() == 0
     host = lib.sa_block_sparse_attn_fwd_host

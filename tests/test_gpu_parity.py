@@ -170,7 +170,8 @@ def _small_case(D, blk, H, nblk, seed, p=0.4):
     return q, k, v, m
 
 
-@pytest.mark.parametrize("D,blk,variant", [(64, 64, 0), (128, 128, 1), (128, 128, 0)])
+@pytest.mark.parametrize("D,blk,variant", [(64, 64, 0), (128, 128, 1), (128, 128, 0), (128, 128, 2),
+                                           (128, 128, 3)])
 def test_small_edge_cases(sa, D, blk, variant):
     # 35 key blocks: two mask words with a ragged tail; n_valid cuts the last block; rows that are
     # empty, full, single-block, only-the-ragged-block; stray bits past NKB; odd row count.
@@ -203,7 +204,7 @@ def test_small_edge_cases(sa, D, blk, variant):
     assert torch.equal(out, out2) and torch.equal(lse, lse2)
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 def test_large_magnitude_scores_and_batch(sa, variant):
     # scores with a wide range (|s| up to ~40): exercises the running-max rescale; B = 2 shares
     # the mask across the batch.
@@ -252,7 +253,7 @@ def test_score_bound_fallbacks(sa, case):
     bits = oracle.pack_bool(m)
     scale = float(np.float32(1 / math.sqrt(D)))
     ref_o, ref_l = oracle.attn(inputs.as_u16(q), inputs.as_u16(k), inputs.as_u16(v), bits, blk, blk, scale)
-    out, lse = run_fwd(sa, q, k, v, bits, blk, scale, variant=0)
+    out, lse = run_fwd(sa, q, k, v, bits, blk, scale, variant=2)     # pair items (the big-problem path)
     # lse is as large as the scores here: 1e-3 absolute is asked of O(10) values (BASELINE.json);
     # allow the fp32 spacing of the value on top (|lse| up to ~1500 -> 1.2e-4 per ulp)
     err = np.abs(lse.cpu().numpy().astype(np.float64) - ref_l)
@@ -263,7 +264,7 @@ def test_score_bound_fallbacks(sa, case):
     assert e.max() <= 4e-2 and e.mean() <= 2e-3, (case, e.max(), e.mean())
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 def test_dense_equals_sdpa_on_gpu_shapes(sa, variant):
     # density 1 ("fully dense setting") at a few-tile size
     D, blk, H, nblk = 128, 128, 2, 6
