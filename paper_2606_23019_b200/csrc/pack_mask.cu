@@ -17,7 +17,7 @@ namespace sa {
 namespace {
 
 constexpr int kHistThreads = 256;
-constexpr int kHistItemsPerBlock = 16384;
+constexpr int kHistRowsPerBlock = 16;     // rows of one head per histogram block (2 per warp)
 
 struct HeadState {      // per head, per pass p = 0..3: state after resolving passes < p
   uint32_t prefix[5];   // high bits fixed so far (prefix[p] has the top 8*p bits set)
@@ -118,14 +118,38 @@ pack_hist_kernel(const float* __restrict__ scores, const float* __restrict__ den
   const uint32_t prefix = s_prefix;
   constexpr int shift = 24 - 8 * PASS;
   const uint32_t hi_mask = PASS == 0 ? 0u : (0xFFFFFFFFu << (32 - 8 * PASS));
-  const size_t total = static_cast<size_t>(NQB) * NKB;
-  const float* sc = scores + static_cast<size_t>(h) * total;
-  const size_t begin = static_cast<size_t>(blockIdx.x) * kHistItemsPerBlock;
-  const size_t end = min(begin + kHistItemsPerBlock, total);
-  for (size_t i = begin + threadIdx.x; i < end; i += blockDim.x) {
-    const int u = static_cast<int>(i / NKB), v = static_cast<int>(i % NKB);
-    const uint32_t key = score_key(__ldg(sc + i), force_diag && u == v);
-    if ((key & hi_mask) == prefix) atomicAdd(&s_hist[(key >> shift) & 0xFFu], 1u);
+  // one warp per row (no index division: the row and column are loop variables), lanes on
+  // consecutive columns (coalesced); equal bins inside a warp are merged before the shared-memory
+  // atomic (the top bytes of real scores take only a handful of values)
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int row0 = blockIdx.x * kHistRowsPerBlock;
+  const int row1 = min(row0 + kHistRowsPerBlock, NQB);
+  for (int u = row0 + warp; u < row1; u += kHistThreads / 32) {
+    const float* row = scores + (static_cast<size_t>(h) * NQB + u) * NKB;
+    for (int v0 = 0; v0 < NKB; v0 += 128) {       // four loads in flight per lane (L2 latency)
+      float x[4];
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const int v = v0 + q * 32 + lane;
+        x[q] = v < NKB ? __ldg(row + v) : 0.f;
+      }
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const int v = v0 + q * 32 + lane;
+        bool hit = false;
+        uint32_t bin = 0u;
+        if (v < NKB) {
+          const uint32_t key = score_key(x[q], force_diag && u == v);
+          hit = (key & hi_mask) == prefix;
+          bin = (key >> shift) & 0xFFu;
+        }
+        const uint32_t active = __ballot_sync(0xFFFFFFFFu, hit);
+        if (hit) {
+          const uint32_t same = __match_any_sync(active, bin);
+          if (lane == __ffs(same) - 1) atomicAdd(&s_hist[bin], static_cast<uint32_t>(__popc(same)));
+        }
+      }
+    }
   }
   __syncthreads();
   uint32_t* hh = hist + (static_cast<size_t>(h) * 4 + PASS) * 256;
@@ -199,8 +223,7 @@ cudaError_t launch_pack_mask(const float* scores, const float* density, uint32_t
   const int W = (NKB + 31) / 32;
   cudaError_t e = cudaMemsetAsync(w.hist, 0, static_cast<size_t>(H) * 4 * 256 * sizeof(uint32_t), st);
   if (e != cudaSuccess) return e;
-  const size_t total = static_cast<size_t>(NQB) * NKB;
-  dim3 hgrid(static_cast<unsigned>((total + kHistItemsPerBlock - 1) / kHistItemsPerBlock), H);
+  dim3 hgrid(static_cast<unsigned>((NQB + kHistRowsPerBlock - 1) / kHistRowsPerBlock), H);
   pack_hist_kernel<0><<<hgrid, kHistThreads, 0, st>>>(scores, density, NQB, NKB, force_diag, w.hist, w.state);
   pack_hist_kernel<1><<<hgrid, kHistThreads, 0, st>>>(scores, density, NQB, NKB, force_diag, w.hist, w.state);
   pack_hist_kernel<2><<<hgrid, kHistThreads, 0, st>>>(scores, density, NQB, NKB, force_diag, w.hist, w.state);
