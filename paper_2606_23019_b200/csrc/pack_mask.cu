@@ -87,18 +87,43 @@ __device__ void resolve(int pass, int h, const float* density, int NQB, int NKB,
   const uint32_t prev_krem = state[h].k_rem[pass - 1];
   if (threadIdx.x < 256) s_suffix[threadIdx.x] = hh[threadIdx.x];
   __syncthreads();
-  if (threadIdx.x == 0) {
-    // walk bins from the largest byte down until the cumulative count reaches k_rem
-    uint32_t above = 0;
-    int bin = 255;
-    for (; bin > 0; --bin) {
-      if (above + s_suffix[bin] >= prev_krem) break;
-      above += s_suffix[bin];
+  if (threadIdx.x < 32) {
+    // bins from the largest byte down until the cumulative count reaches k_rem: lane l owns the 8
+    // bins 255-8l .. 248-8l; a warp scan gives the count above each lane's group
+    const int lane = threadIdx.x;
+    uint32_t c[8], sum = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      c[i] = s_suffix[255 - 8 * lane - i];
+      sum += c[i];
     }
-    const int shift = 32 - 8 * pass;
-    *s_prefix = prev_prefix | (static_cast<uint32_t>(bin) << shift);
-    *s_krem = prev_krem - above;
-    if (record) { state[h].prefix[pass] = *s_prefix; state[h].k_rem[pass] = *s_krem; }
+    uint32_t incl = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t t = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+      if (lane >= o) incl += t;
+    }
+    uint32_t above = incl - sum;                       // keys in bins above this lane's group
+    const bool here = above < prev_krem && incl >= prev_krem;
+    const uint32_t who = __ballot_sync(0xFFFFFFFFu, here);
+    // nobody reaches k_rem (cannot happen for a consistent histogram): fall to bin 0 like the walk
+    const int owner = who ? __ffs(who) - 1 : 31;
+    if (lane == owner) {
+      int bin = 255 - 8 * lane;
+      int i = 0;
+      for (; i < 7; ++i, --bin) {
+        if (above + c[i] >= prev_krem) break;
+        above += c[i];
+      }
+      if (!who) {                                      // walk semantics: stop at bin 0 whatever it holds
+        bin = 0;
+        above = incl - c[7];
+      }
+      const int shift = 32 - 8 * pass;
+      *s_prefix = prev_prefix | (static_cast<uint32_t>(bin) << shift);
+      *s_krem = prev_krem - above;
+      if (record) { state[h].prefix[pass] = *s_prefix; state[h].k_rem[pass] = *s_krem; }
+    }
   }
   __syncthreads();
 }
