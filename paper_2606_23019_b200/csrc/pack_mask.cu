@@ -144,8 +144,7 @@ pack_hist_kernel(const float* __restrict__ scores, const float* __restrict__ den
   constexpr int shift = 24 - 8 * PASS;
   const uint32_t hi_mask = PASS == 0 ? 0u : (0xFFFFFFFFu << (32 - 8 * PASS));
   // one warp per row (no index division: the row and column are loop variables), lanes on
-  // consecutive columns (coalesced); equal bins inside a warp are merged before the shared-memory
-  // atomic (the top bytes of real scores take only a handful of values)
+  // consecutive columns (coalesced)
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int row0 = blockIdx.x * kHistRowsPerBlock;
   const int row1 = min(row0 + kHistRowsPerBlock, NQB);
@@ -168,10 +167,14 @@ pack_hist_kernel(const float* __restrict__ scores, const float* __restrict__ den
           hit = (key & hi_mask) == prefix;
           bin = (key >> shift) & 0xFFu;
         }
-        const uint32_t active = __ballot_sync(0xFFFFFFFFu, hit);
-        if (hit) {
-          const uint32_t same = __match_any_sync(active, bin);
-          if (lane == __ffs(same) - 1) atomicAdd(&s_hist[bin], static_cast<uint32_t>(__popc(same)));
+        if (PASS == 0) {           // top byte: a handful of values -> merge equal bins in the warp
+          const uint32_t active = __ballot_sync(0xFFFFFFFFu, hit);
+          if (hit) {
+            const uint32_t same = __match_any_sync(active, bin);
+            if (lane == __ffs(same) - 1) atomicAdd(&s_hist[bin], static_cast<uint32_t>(__popc(same)));
+          }
+        } else if (hit) {          // lower bytes: bins are spread (match.any would loop per value)
+          atomicAdd(&s_hist[bin], 1u);
         }
       }
     }
