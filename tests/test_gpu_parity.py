@@ -322,6 +322,15 @@ def test_c2_full_size_sampled_units_and_variant_agreement(sa):
     assert abs(dense.mean() - 0.25) < 0.1
 
 
+def test_c3_full_size_sampled_units(sa):
+    # BASELINE.json configs[2]: Wan2.1-14B 480p shapes, per-head density U(0.05, 0.35)
+    cfg = inputs.C3
+    q, k, v, bits, bits_t = _full_size_inputs(sa, cfg)
+    _, _, dense = _sampled_unit_parity(sa, cfg, q, k, v, bits, bits_t, variant=0, n_heads=4)
+    per_head = dense.reshape(cfg.H, -1).mean(axis=1)
+    assert 0.04 < per_head.min() < 0.12 and 0.28 < per_head.max() < 0.36     # uneven heads
+
+
 def test_c4_full_size_sampled_units(sa):
     # the configuration bench.py times (Wan2.1-14B 720p shapes), same launch path
     cfg = inputs.C4
