@@ -337,27 +337,6 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
   while (npend > 0) pop();
 }
 
-// 2^x for two lanes on the FMA pipe (no MUFU): x = n + f with n = floor(x) (round-down add of
-// 1.5*2^23 leaves n in the low mantissa bits), 2^f by a degree-3 polynomial with p(0) = 1 (max
-// relative error 8.6e-5 on [0,1), mean +7e-6 -- below the bf16 rounding of P), and n added to the
-// exponent field by one shift-add. x is clamped at -127 so the exponent cannot wrap.
-__device__ __forceinline__ void exp2_fma_pipe(uint64_t x, float& e0, float& e1) {
-  float x0, x1;
-  up2(x, x0, x1);
-  const uint64_t xc = pk2(fmaxf(x0, -127.f), fmaxf(x1, -127.f));
-  const uint64_t magic = pk2(12582912.f, 12582912.f);
-  const uint64_t r = add2_rm(xc, magic);
-  const uint64_t f = sub2(xc, sub2(r, magic));
-  uint64_t q = fma2(f, pk2(0.07706704f, 0.07706704f), pk2(0.22764499f, 0.22764499f));
-  q = fma2(q, f, pk2(0.69511676f, 0.69511676f));
-  q = fma2(q, f, pk2(1.f, 1.f));
-  float q0, q1, r0, r1;
-  up2(q, q0, q1);
-  up2(r, r0, r1);
-  e0 = __int_as_float(__float_as_int(q0) + (__float_as_int(r0) << 23));
-  e1 = __int_as_float(__float_as_int(q1) + (__float_as_int(r1) << 23));
-}
-
 // P = 2^(c*s - m) of one query row (128 columns in sr), written to TMEM as bf16 in kPChunks pieces
 // (p_full[piece] arrives after each); returns the row sum. Packed FFMA2 for the argument; of every
 // 4 column pairs NPOLY take the FMA-pipe exp2 and the rest MUFU.EX2 (the ragged tile uses

@@ -30,6 +30,11 @@ constexpr uint32_t kTileBytes = kBlk * kD * 2;      // 32 KB
 constexpr uint32_t kHalfBytes = kTileBytes / 2;
 constexpr int kSlots = 6;                           // K ring
 constexpr uint32_t kTmemCols = 256;                 // two fp32 128 x 128 S buffers
+#ifndef SA_SIG_POLY_PAIRS
+#define SA_SIG_POLY_PAIRS 1
+#endif
+constexpr int kSigPolyPairs = SA_SIG_POLY_PAIRS;    // of every 4 column pairs, how many take exp2 on the FMA pipe
+                                                    // (measured at C3: 0 -> 12.94 ms, 1 -> 12.32 ms, 2 -> 14.36 ms)
 
 constexpr uint32_t kOffQ = 0;
 constexpr uint32_t kOffRing = kTileBytes;
@@ -159,10 +164,18 @@ __device__ void sum_wg(const SigParams& p, Ctl* ctl, uint32_t tmem, int g, int q
         for (int cc = 0; cc < 4; ++cc)
 #pragma unroll
           for (int i = 0; i < 16; ++i) {
-            float x0, x1;
-            up2(fma2(pk2(__uint_as_float(sr[cc][2 * i]), __uint_as_float(sr[cc][2 * i + 1])), c2, nl22),
-                x0, x1);
-            acc[i & 3] = add2(acc[i & 3], pk2(ex2(x0), ex2(x1)));
+            const uint64_t x = fma2(pk2(__uint_as_float(sr[cc][2 * i]), __uint_as_float(sr[cc][2 * i + 1])),
+                                    c2, nl22);
+            float e0, e1;
+            if ((i & 3) < kSigPolyPairs) {             // FMA-pipe exp2: this kernel is MUFU-bound
+              exp2_fma_pipe(x, e0, e1);
+            } else {
+              float x0, x1;
+              up2(x, x0, x1);
+              e0 = ex2(x0);
+              e1 = ex2(x1);
+            }
+            acc[i & 3] = add2(acc[i & 3], pk2(e0, e1));
           }
       } else {                                                    // the ragged tail tile
 #pragma unroll
