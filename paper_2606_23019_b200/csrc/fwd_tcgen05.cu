@@ -45,6 +45,7 @@ constexpr uint32_t kTileBytes = kBlk * kD * 2;      // 32 KB
 constexpr uint32_t kHalfBytes = kTileBytes / 2;     // one [128][64] swizzle-128B box
 constexpr int kSlots = 5;                 // K/V ring
 constexpr int kSched = 2;                 // scheduler ring
+constexpr int kClaimAheadUnits = 512;     // items up to this many (tile, key block) units claim their successor early
 constexpr uint32_t kTmemCols = 512;
 constexpr float kRescaleThreshold = 8.0f; // log2 units
 constexpr float kBoundSlack = 64.0f;      // log2 units: how far the Cauchy-Schwarz bound may lie above
@@ -140,21 +141,38 @@ __device__ void producer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, const
   Ring ring;
   uint32_t q_phase = 0;
   int sched_n = 0;
-  for (;;) {
+  // Work items are claimed ONE AHEAD: while the loads of item n are issued, item n+1 has already
+  // been taken from the list and published in the 2-slot scheduler ring, so that at the end of an
+  // item nobody waits for the atomic and the list lookup (two dependent global round trips, ~3 us
+  // of idle tensor pipe per item otherwise). The list is longest-first inside a head, so the items
+  // claimed early near the end are the light ones and the tail stays short.
+  auto claim_and_publish = [&]() {
     int idx = 0;
     if (lane == 0) idx = atomicAdd(p.counter, 1);
     idx = __shfl_sync(0xFFFFFFFFu, idx, 0);
-    const int item = idx < p.n_items ? __ldg(p.unit_order + idx) : -1;
+    const int it_id = idx < p.n_items ? __ldg(p.unit_order + idx) : -1;
     const int ss = sched_n % kSched;
     mbar_wait(smem_u32(&ctl->sched_empty[ss]), ((sched_n / kSched) & 1) ^ 1u, 1);
     if (lane == 0) {
-      ctl->sched_item[ss] = item;
+      ctl->sched_item[ss] = it_id;
       mbar_arrive(smem_u32(&ctl->sched_full[ss]));
     }
     __syncwarp();
     ++sched_n;
+    return it_id;
+  };
+  int next_item = claim_and_publish();
+  for (;;) {
+    const int item = next_item;
     if (item < 0) break;
     const Item it = decode_item(p, item, items_per_head);
+    // ... unless this item is a long one (a held-back item would then wait that long while another
+    // CTA may be idle): long items claim their successor only when their own loads are out
+    int units = 0;
+    for (int w = 0; w < p.W; ++w)
+      units += __popc(row_word(p, it.h, it.u0, w, true)) + __popc(row_word(p, it.h, it.u0 + 1, w, it.has1));
+    const bool ahead = units <= kClaimAheadUnits;
+    if (ahead) next_item = claim_and_publish();
 
     mbar_wait(smem_u32(&ctl->q_empty), q_phase ^ 1u, 2);
     const uint32_t qf = smem_u32(&ctl->q_full);
@@ -186,6 +204,7 @@ __device__ void producer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, const
         }
       }
     }
+    if (!ahead) next_item = claim_and_publish();
   }
   // every MMA that reads shared memory has retired before the CTA exits
   mbar_wait(smem_u32(&ctl->q_empty), q_phase ^ 1u, 4);
