@@ -8,7 +8,10 @@
 // How (this design is for B200, not the paper's):
 //   * persistent grid, one CTA per SM; a work item is a PAIR of adjacent query blocks (2u, 2u+1)
 //     of one (batch, head). Items are pulled from the popcount-ordered list of the schedule
-//     pre-pass with an atomic cursor, so uneven rows and heads balance out.
+//     pre-pass with an atomic cursor, so uneven rows and heads balance out. The producer claims
+//     one item ahead (2-slot scheduler ring) so the atomic's round trip hides under the current
+//     item's loads; after a long item the claim is taken late instead, so that the tail of the
+//     grid still goes to whichever CTA is free first.
 //   * the two query tiles have different bit-rows; the CTA walks the UNION of the two rows, stages
 //     each K/V tile of the union ONCE (TMA, 128B swizzle, 5-slot ring of 32 KB tiles), and issues
 //     the MMAs of a tile only where that tile's own bit is set, so a key block both rows have is
