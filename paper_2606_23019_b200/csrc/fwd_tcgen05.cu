@@ -70,6 +70,7 @@ constexpr int kPolyPairs = SA_POLY_PAIRS;
 constexpr int kPChunks = SA_PCHUNKS;
 static_assert(kPolyPairs >= 0 && kPolyPairs <= 4, "SA_POLY_PAIRS in 0..4");
 static_assert(kPChunks == 1 || kPChunks == 2 || kPChunks == 4, "SA_PCHUNKS in {1,2,4}");
+static_assert(kPChunks == 2, "the MMA issuer takes P in two pieces");
 
 // shared memory map (offsets from a 1024 B aligned base)
 constexpr uint32_t kOffQ = 0;                                   // 2 query tiles
@@ -214,39 +215,26 @@ __device__ void producer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, const
 }
 
 // ------------------------------------------------------------------ warp 1: MMA issuer
-__device__ __forceinline__ void issue_qk(uint32_t tmem_s, uint32_t q_addr, uint32_t k_addr) {
-#pragma unroll
-  for (int kk = 0; kk < kD / 16; ++kk) {
-    const uint32_t off = (kk >> 2) * kHalfBytes + (kk & 3) * 32;
-    mma_ss_e(tmem_s, make_desc(kDescKMajor, q_addr + off), make_desc(kDescKMajor, k_addr + off),
-             kIdescQK, kk > 0);
-  }
-}
-// P arrives in kPChunks pieces (p_full[c], c ascending); the MMAs of a piece are issued as soon as
-// that piece is in TMEM.
-__device__ __forceinline__ void issue_pv(uint32_t tmem_o, uint32_t tmem_p, uint32_t v_addr,
-                                         bool accumulate, const uint64_t* p_full, uint32_t phase) {
-  constexpr int kPer = (kBlk / 16) / kPChunks;
-#pragma unroll
-  for (int kk = 0; kk < kBlk / 16; ++kk) {
-    if (kk % kPer == 0) {
-      mbar_wait(smem_u32(&p_full[kk / kPer]), phase, 13);
-      tc_fence_after();
-    }
-    mma_ts_e(tmem_o, tmem_p + kk * 8, make_desc(kDescMNMajor, v_addr + kk * 16 * 128), kIdescPV,
-             accumulate || kk > 0);
-  }
-}
+#ifdef SA_TRACE
+#define IT_TR(i) { const uint32_t n_ = clock(); itr[i] += n_ - itl; itl = n_; }
+#else
+#define IT_TR(i)
+#endif
 
-// One (query tile, key block) unit whose S has been issued and whose PV is still to come.
+// One (query tile, key block) unit whose S has been issued and whose PV is still to come. Every
+// address and descriptor is worked out when the unit is created, BEFORE the issuer blocks on the
+// older unit's P: once P is there, nothing but waits, MMAs and commits lies between it and the
+// next S (the MMA issuer is a serial resource inside the cycle S -> softmax -> PV -> next S).
 struct Pend {
-  uint32_t t, buf;             // tile, S/P buffer in TMEM
-  uint32_t sel, par;           // this unit's barriers: [t][sel], phase parity par
-  uint32_t vslot, vphase;      // ring slot holding V and the parity of its kv_full
+  uint32_t tmem_o, tmem_p;     // O_t and the unit's P (first columns of its S/P buffer)
+  uint64_t vdesc;              // V tile as the MN-major B operand
   uint32_t acc;                // accumulate into O_t (0 for the tile's first unit of the item)
-  uint32_t ofree_par;          // first unit only: parity of o_free[t] to wait for
-  uint32_t last_of_tile;       // last unit of this tile in its item: commit o_full[t] after the PV
-  uint32_t rel_v;              // last user of the V slot: release it after the PV
+  uint32_t p_full, par;        // p_full[t][sel][0] (piece c at + 8 c) and its phase parity
+  uint32_t pv_done;            // barrier committed after the PV
+  uint32_t v_full, vphase;     // ring slot holding V: kv_full and its parity
+  uint32_t o_free, ofree_par;  // first unit of a tile only (else 0): wait before overwriting O_t
+  uint32_t v_empty;            // last user of the V slot (else 0): release it after the PV
+  uint32_t o_full;             // last unit of the tile in its item (else 0): commit after the PV
 };
 
 // Runs on every lane of warp 1 (converged); elect.sync inside the _e wrappers picks the issuer.
@@ -266,17 +254,30 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
   int sched_n = 0;
   Pend pd0{}, pd1{};                     // FIFO: pd0 older
   int npend = 0;
+  auto bar = [&](const void* b) { return smem_u32(b); };
+#ifdef SA_TRACE
+  uint32_t itr[7] = {0, 0, 0, 0, 0, 0, 0}, itl = clock(), it_units = 0;
+#endif
 
+  // P arrives in two pieces (p_full + 8 c): the MMAs of a piece are issued as soon as it is in TMEM
   auto issue_pend = [&](const Pend& u) {
-    if (!u.acc) mbar_wait(smem_u32(&ctl->o_free[u.t]), u.ofree_par, 12);
-    mbar_wait(smem_u32(&ctl->kv_full[u.vslot]), u.vphase, 15);
+    IT_TR(0);
+    if (u.o_free) mbar_wait(u.o_free, u.ofree_par, 12);
+    mbar_wait(u.v_full, u.vphase, 15);
+    IT_TR(3);
+    mbar_wait(u.p_full, u.par, 13);
     tc_fence_after();
-    issue_pv(tmem + 256 + u.t * 128, tmem + u.buf * 128,
-             smem_base + kOffRing + u.vslot * kTileBytes, u.acc != 0, ctl->p_full[u.t][u.sel],
-             u.par);
-    tc_commit_e(smem_u32(&ctl->pv_done[u.t][u.sel]));
-    if (u.rel_v) tc_commit_e(smem_u32(&ctl->kv_empty[u.vslot]));
-    if (u.last_of_tile) tc_commit_e(smem_u32(&ctl->o_full[u.t]));
+    IT_TR(1);
+    mma_ts_e4<8, 128>(u.tmem_o, u.tmem_p, u.vdesc, kIdescPV, u.acc);
+    IT_TR(6);
+    mbar_wait(u.p_full + 8, u.par, 13);
+    tc_fence_after();
+    IT_TR(1);
+    mma_ts_e4<8, 128>(u.tmem_o, u.tmem_p + 32, u.vdesc + 4 * 128, kIdescPV, 1u);
+    tc_commit_e(u.pv_done);
+    if (u.v_empty) tc_commit_e(u.v_empty);
+    if (u.o_full) tc_commit_e(u.o_full);
+    IT_TR(6);
   };
   auto pop = [&]() {
     issue_pend(pd0);
@@ -286,8 +287,11 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
 
   for (;;) {
     const int ss = sched_n % kSched;
+    IT_TR(0);
     mbar_wait(smem_u32(&ctl->sched_full[ss]), (sched_n / kSched) & 1, 10);
-    const int item = ctl->sched_item[ss];
+    IT_TR(4);
+    // warp-uniform by construction; the reduction tells the compiler so (see uni())
+    const int item = static_cast<int>(uni(static_cast<uint32_t>(ctl->sched_item[ss])));
     __syncwarp();
     if (lane == 0) mbar_arrive(smem_u32(&ctl->sched_empty[ss]));
     ++sched_n;
@@ -296,8 +300,8 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
 
     uint32_t rem[2] = {0, 0};            // units each tile still has in this item
     for (int w = 0; w < p.W; ++w) {
-      rem[0] += __popc(row_word(p, it.h, it.u0, w, true));
-      rem[1] += __popc(row_word(p, it.h, it.u0 + 1, w, it.has1));
+      rem[0] += __popc(uni(row_word(p, it.h, it.u0, w, true)));
+      rem[1] += __popc(uni(row_word(p, it.h, it.u0 + 1, w, it.has1)));
     }
     bool first[2] = {true, true};
 
@@ -306,57 +310,119 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     // is not there yet, issue the parked PVs first (they need nothing from the next item).
     if (!mbar_try_wait(smem_u32(&ctl->q_full), q_phase))
       while (npend > 0) pop();
+    IT_TR(0);
     mbar_wait(smem_u32(&ctl->q_full), q_phase, 11);
+    IT_TR(4);
     q_phase ^= 1u;
     tc_fence_after();
-    for (int w = 0; w < p.W; ++w) {
-      const uint32_t x0 = row_word(p, it.h, it.u0, w, true);
-      const uint32_t x1 = row_word(p, it.h, it.u0 + 1, w, it.has1);
-      uint32_t x = x0 | x1;
-      while (x) {
-        const int bit = __ffs(x) - 1;
-        x &= x - 1u;
-        const bool has[2] = {((x0 >> bit) & 1u) != 0, ((x1 >> bit) & 1u) != 0};
-        const int kslot = ring.slot;
-        const uint32_t kphase = ring.phase;
-        ring.advance();
-        const uint32_t vslot = ring.slot;
-        const uint32_t vphase = ring.phase;
-        ring.advance();
-        const uint32_t k_addr = smem_base + kOffRing + kslot * kTileBytes;
-        if (npend == 2) pop();             // the oldest PV does not need this block's K: issue it first
-        mbar_wait(smem_u32(&ctl->kv_full[kslot]), kphase, 14);
-        tc_fence_after();
-#pragma unroll
-        for (int t = 0; t < 2; ++t) {
-          if (!has[t]) continue;
-          if (npend == 2) pop();
-          Pend u;
-          u.t = t;
-          u.buf = wg & 1u;
-          u.sel = nt[t] & 1u;
-          u.par = (nt[t] >> 1) & 1u;
-          ++nt[t];
-          u.vslot = vslot;
-          u.vphase = vphase;
-          u.acc = first[t] ? 0u : 1u;
-          u.ofree_par = (n_started[t] & 1u) ^ 1u;
-          u.last_of_tile = (--rem[t] == 0u) ? 1u : 0u;
-          u.rel_v = (t == 1 || !has[1]) ? 1u : 0u;
-          if (first[t]) ++n_started[t];
-          first[t] = false;
-          issue_qk(tmem + u.buf * 128, smem_base + kOffQ + t * kTileBytes, k_addr);
-          tc_commit_e(smem_u32(&ctl->s_full[t][u.sel]));
-          if (npend == 0) pd0 = u; else pd1 = u;
-          ++npend;
-          ++wg;
+    // Key blocks of the union, one ahead: the next block's bookkeeping (mask walk, ring slots,
+    // descriptors) is done right after the first half of the current block's last S has been
+    // issued, i.e. while the tensor pipe still has those MMAs queued, not between two units.
+    struct Blk {
+      bool valid, has0, has1;
+      uint32_t k_full, kphase, k_empty, v_full, vphase, v_empty;
+      uint64_t kdesc, vdesc;
+    };
+    int bw = -1;                         // word index of the walk
+    uint32_t bx = 0, bx0 = 0, bx1 = 0;   // bits left in the word, the two rows' words
+    uint32_t nx0 = row_word(p, it.h, it.u0, 0, true), nx1 = row_word(p, it.h, it.u0 + 1, 0, it.has1);
+    auto next_blk = [&]() {
+      Blk b;
+      b.valid = false;
+      while (bx == 0u) {
+        if (++bw >= p.W) return b;
+        bx0 = uni(nx0);
+        bx1 = uni(nx1);
+        if (bw + 1 < p.W) {              // the mask words are fetched one word ahead
+          nx0 = row_word(p, it.h, it.u0, bw + 1, true);
+          nx1 = row_word(p, it.h, it.u0 + 1, bw + 1, it.has1);
         }
-        tc_commit_e(smem_u32(&ctl->kv_empty[kslot]));
+        bx = bx0 | bx1;
       }
+      const int bit = __ffs(bx) - 1;
+      bx &= bx - 1u;
+      b.valid = true;
+      b.has0 = ((bx0 >> bit) & 1u) != 0;
+      b.has1 = ((bx1 >> bit) & 1u) != 0;
+      const int kslot = ring.slot;
+      b.kphase = ring.phase;
+      ring.advance();
+      const int vslot = ring.slot;
+      b.vphase = ring.phase;
+      ring.advance();
+      b.k_full = bar(&ctl->kv_full[kslot]);
+      b.k_empty = bar(&ctl->kv_empty[kslot]);
+      b.v_full = bar(&ctl->kv_full[vslot]);
+      b.v_empty = bar(&ctl->kv_empty[vslot]);
+      b.kdesc = make_desc(kDescKMajor, smem_base + kOffRing + kslot * kTileBytes);
+      b.vdesc = make_desc(kDescMNMajor, smem_base + kOffRing + vslot * kTileBytes);
+      return b;
+    };
+    Blk cb = next_blk();
+    while (cb.valid) {
+      Blk nb;
+      nb.valid = false;
+      bool k_ready = false;
+#pragma unroll
+      for (int t = 0; t < 2; ++t) {
+        if (!(t == 0 ? cb.has0 : cb.has1)) continue;
+        const bool last_of_blk = t == 1 || !cb.has1;
+        // everything the unit needs, before the issuer blocks on the oldest unit's P
+        Pend u;
+        const uint32_t buf = wg & 1u, sel = nt[t] & 1u;
+        u.tmem_o = tmem + 256 + t * 128;
+        u.tmem_p = tmem + buf * 128;
+        u.vdesc = cb.vdesc;
+        u.acc = first[t] ? 0u : 1u;
+        u.p_full = bar(&ctl->p_full[t][sel][0]);
+        u.par = (nt[t] >> 1) & 1u;
+        u.pv_done = bar(&ctl->pv_done[t][sel]);
+        u.v_full = cb.v_full;
+        u.vphase = cb.vphase;
+        u.o_free = first[t] ? bar(&ctl->o_free[t]) : 0u;
+        u.ofree_par = (n_started[t] & 1u) ^ 1u;
+        u.v_empty = last_of_blk ? cb.v_empty : 0u;
+        u.o_full = (--rem[t] == 0u) ? bar(&ctl->o_full[t]) : 0u;
+        const uint32_t tmem_s = tmem + buf * 128;
+        const uint64_t qdesc = make_desc(kDescKMajor, smem_base + kOffQ + t * kTileBytes);
+        const uint32_t s_full = bar(&ctl->s_full[t][sel]);
+        ++nt[t];
+        if (first[t]) ++n_started[t];
+        first[t] = false;
+        ++wg;
+        if (!k_ready) k_ready = mbar_try_wait(cb.k_full, cb.kphase);
+        if (npend == 2) pop();           // PV of the oldest unit: it frees this unit's S buffer
+        if (!k_ready) {
+          IT_TR(0);
+          mbar_wait(cb.k_full, cb.kphase, 14);
+          IT_TR(2);
+          k_ready = true;
+        }
+        tc_fence_after();
+        IT_TR(0);
+        mma_ss_e4<2, 2>(tmem_s, qdesc, cb.kdesc, kIdescQK, 0u);
+        if (last_of_blk) nb = next_blk();
+        mma_ss_e4<2, 2>(tmem_s, qdesc + (kHalfBytes >> 4), cb.kdesc + (kHalfBytes >> 4), kIdescQK, 1u);
+        tc_commit_e(s_full);
+        IT_TR(5);
+#ifdef SA_TRACE
+        ++it_units;
+#endif
+        if (npend == 0) pd0 = u; else pd1 = u;
+        ++npend;
+      }
+      tc_commit_e(cb.k_empty);
+      cb = nb;
     }
     tc_commit_e(smem_u32(&ctl->q_empty));   // every S of this item has been issued
   }
   while (npend > 0) pop();
+#ifdef SA_TRACE
+  if (lane == 0 && blockIdx.x < 2)
+    printf("issuer cta %d units %u: other %u | p_full %u | K %u | V/o_free %u | sched/q %u | S issue %u | PV issue %u (clk per unit)\n",
+           blockIdx.x, it_units, itr[0] / it_units, itr[1] / it_units, itr[2] / it_units, itr[3] / it_units,
+           itr[4] / it_units, itr[5] / it_units, itr[6] / it_units);
+#endif
 }
 
 // P = 2^(c*s - m) of one query row (128 columns in sr), written to TMEM as bf16 in kPChunks pieces
@@ -475,18 +541,26 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     bool started = false;
     bool fixed = false;                  // warp-uniform: m_run is the bound, fixed for the item
     uint32_t prev_unit = 0xFFFFFFFEu;    // this tile's previous unit in the item
-    // walk the union of the two bit-rows (the unit numbering needs both), handle this tile's units
+    // Walk this tile's own bit-row. A unit's number in the union walk order (which the MMA issuer
+    // follows) is the popcount of both rows below its bit. The mask words are fetched one word
+    // ahead and the next unit's bookkeeping is computed in the same straight-line block as the
+    // exponentials, so neither sits in the cycle S -> softmax -> PV -> next S.
+    uint32_t nx0 = row_word(p, it.h, it.u0, 0, true), nx1 = row_word(p, it.h, it.u0 + 1, 0, it.has1);
     for (int w = 0; w < p.W; ++w) {
-      const uint32_t x0 = row_word(p, it.h, it.u0, w, true);
-      const uint32_t x1 = row_word(p, it.h, it.u0 + 1, w, it.has1);
-      uint32_t x = x0 | x1;
-      while (x) {
-        const int bit = __ffs(x) - 1;
-        x &= x - 1u;
-        const uint32_t a = (x0 >> bit) & 1u, b = (x1 >> bit) & 1u;
-        const uint32_t my = wg + (t == 1 ? a : 0u);
-        wg += a + b;
-        if (!(t == 0 ? a : b)) continue;
+      const uint32_t x0 = nx0, x1 = nx1;
+      if (w + 1 < p.W) {
+        nx0 = row_word(p, it.h, it.u0, w + 1, true);
+        nx1 = row_word(p, it.h, it.u0 + 1, w + 1, it.has1);
+      }
+      uint32_t xm = t == 0 ? x0 : x1;
+      const uint32_t wbase = wg;
+      wg += __popc(x0) + __popc(x1);
+      if (!xm) continue;
+      int bit = __ffs(xm) - 1;
+      xm &= xm - 1u;
+      uint32_t my = wbase + __popc(x0 & ((1u << bit) - 1u)) + __popc(x1 & ((1u << bit) - 1u)) +
+                    (t == 1 ? (x0 >> bit) & 1u : 0u);
+      for (;;) {
         const int j = w * 32 + bit;
         const uint32_t buf = my & 1u, sel = nmine & 1u, par = (nmine >> 1) & 1u;
         const uint32_t tm_s = tmem + lane_base + buf * 128;
@@ -555,12 +629,21 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
         }
         const float m_use = (m_run == -INFINITY) ? 0.f : m_run;
         SA_TR(3);
+        // this tile's next unit in the word, if any (nbit = -1 -> the values are not used)
+        const bool more = xm != 0u;
+        const int nbit = (__ffs(xm) - 1) & 31;
+        xm &= xm - 1u;
+        const uint32_t nmy = wbase + __popc(x0 & ((1u << nbit) - 1u)) + __popc(x1 & ((1u << nbit) - 1u)) +
+                             (t == 1 ? (x0 >> nbit) & 1u : 0u);
         if (ragged) l_run += exp_tile<0>(sr, c, m_use, tm_s, ctl->p_full[t][sel], lane);
         else l_run += exp_tile<kPolyPairs>(sr, c, m_use, tm_s, ctl->p_full[t][sel], lane);
         SA_TR(4);
         started = true;
         prev_unit = my;
         ++nmine;
+        if (!more) break;
+        bit = nbit;
+        my = nmy;
       }
     }
 
@@ -614,7 +697,8 @@ fwd_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
   const uint32_t raw = smem_u32(smem_raw);
   const uint32_t smem_base = (raw + 1023u) & ~1023u;
   Ctl* ctl = reinterpret_cast<Ctl*>(smem_raw + (smem_base - raw) + kOffCtl);
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  // warp index through a shuffle: the compiler then knows it is warp-uniform, and so is the role branch
+  const int warp = __shfl_sync(0xFFFFFFFFu, static_cast<int>(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
   const int items_per_head = (p.NQB + p.rows_per_item - 1) / p.rows_per_item;
 
   if (threadIdx.x == 0) {

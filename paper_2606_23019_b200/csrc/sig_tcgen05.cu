@@ -209,7 +209,9 @@ sig_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
   const uint32_t smem_base = smem_u32(smem_raw);
   if (smem_base & 1023u) __trap();   // 128B-swizzled TMA / UMMA tiles need a 1024 B aligned base
   Ctl* ctl = reinterpret_cast<Ctl*>(smem_raw + kOffCtl);
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  // warp index through a shuffle: the compiler then knows it is warp-uniform, and the role code below runs on the
+  // uniform datapath (see fwd_tcgen05.cu)
+  const int warp = __shfl_sync(0xFFFFFFFFu, static_cast<int>(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
   if (threadIdx.x == 0) {
     prefetch_tensormap(&tm_q);
     prefetch_tensormap(&tm_k);
