@@ -129,6 +129,33 @@ __device__ __forceinline__ uint32_t row_word(const FwdParams& p, int h, int u, i
   return x;
 }
 
+// The two bit-rows of a work item, held by the warp: lane l keeps words (base + l) and (base + 32 + l)
+// of each row, fetched with one coalesced load per 64 words; word w is then a shuffle away instead of
+// a dependent global load per word (at low density most words hold 0-2 key blocks, and a load per
+// word put an L2 round trip into every role's walk). The shuffle's source lane is warp-uniform, so
+// the result is too.
+struct RowWalk {
+  uint32_t a0 = 0, a1 = 0, b0 = 0, b1 = 0;
+  __device__ __forceinline__ void load(const FwdParams& p, const Item& it, int base, int lane) {
+    const int w0 = base + lane, w1 = base + 32 + lane;
+    a0 = w0 < p.W ? row_word(p, it.h, it.u0, w0, true) : 0u;
+    a1 = w1 < p.W ? row_word(p, it.h, it.u0, w1, true) : 0u;
+    b0 = w0 < p.W ? row_word(p, it.h, it.u0 + 1, w0, it.has1) : 0u;
+    b1 = w1 < p.W ? row_word(p, it.h, it.u0 + 1, w1, it.has1) : 0u;
+  }
+  // number of set bits of each row within the loaded 64 words
+  __device__ __forceinline__ void counts(uint32_t& n0, uint32_t& n1) const {
+    n0 = __reduce_add_sync(0xFFFFFFFFu, __popc(a0) + __popc(a1));
+    n1 = __reduce_add_sync(0xFFFFFFFFu, __popc(b0) + __popc(b1));
+  }
+  __device__ __forceinline__ uint32_t row0(int w) const {
+    return __shfl_sync(0xFFFFFFFFu, (w & 32) ? a1 : a0, w & 31);
+  }
+  __device__ __forceinline__ uint32_t row1(int w) const {
+    return __shfl_sync(0xFFFFFFFFu, (w & 32) ? b1 : b0, w & 31);
+  }
+};
+
 struct Ring {
   int slot = 0;
   uint32_t phase = 0;
@@ -172,10 +199,15 @@ __device__ void producer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, const
     const Item it = decode_item(p, item, items_per_head);
     // ... unless this item is a long one (a held-back item would then wait that long while another
     // CTA may be idle): long items claim their successor only when their own loads are out
-    int units = 0;
-    for (int w = 0; w < p.W; ++w)
-      units += __popc(row_word(p, it.h, it.u0, w, true)) + __popc(row_word(p, it.h, it.u0 + 1, w, it.has1));
-    const bool ahead = units <= kClaimAheadUnits;
+    RowWalk rw;
+    uint32_t units = 0;
+    for (int base = 0; base < p.W; base += 64) {
+      uint32_t n0, n1;
+      rw.load(p, it, base, lane);
+      rw.counts(n0, n1);
+      units += n0 + n1;
+    }
+    const bool ahead = units <= static_cast<uint32_t>(kClaimAheadUnits);
     if (ahead) next_item = claim_and_publish();
 
     mbar_wait(smem_u32(&ctl->q_empty), q_phase ^ 1u, 2);
@@ -190,7 +222,8 @@ __device__ void producer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, const
     q_phase ^= 1u;
 
     for (int w = 0; w < p.W; ++w) {
-      uint32_t x = row_word(p, it.h, it.u0, w, true) | row_word(p, it.h, it.u0 + 1, w, it.has1);
+      if ((w & 63) == 0 && (w > 0 || p.W > 64)) rw.load(p, it, w, lane);
+      uint32_t x = rw.row0(w) | rw.row1(w);
       while (x) {
         const int j = w * 32 + (__ffs(x) - 1);
         x &= x - 1u;
@@ -298,10 +331,14 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     if (item < 0) break;
     const Item it = decode_item(p, item, items_per_head);
 
+    RowWalk rw;
     uint32_t rem[2] = {0, 0};            // units each tile still has in this item
-    for (int w = 0; w < p.W; ++w) {
-      rem[0] += __popc(uni(row_word(p, it.h, it.u0, w, true)));
-      rem[1] += __popc(uni(row_word(p, it.h, it.u0 + 1, w, it.has1)));
+    for (int base = 0; base < p.W; base += 64) {
+      uint32_t n0, n1;
+      rw.load(p, it, base, lane);
+      rw.counts(n0, n1);
+      rem[0] += n0;
+      rem[1] += n1;
     }
     bool first[2] = {true, true};
 
@@ -325,18 +362,14 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     };
     int bw = -1;                         // word index of the walk
     uint32_t bx = 0, bx0 = 0, bx1 = 0;   // bits left in the word, the two rows' words
-    uint32_t nx0 = row_word(p, it.h, it.u0, 0, true), nx1 = row_word(p, it.h, it.u0 + 1, 0, it.has1);
     auto next_blk = [&]() {
       Blk b;
       b.valid = false;
       while (bx == 0u) {
         if (++bw >= p.W) return b;
-        bx0 = uni(nx0);
-        bx1 = uni(nx1);
-        if (bw + 1 < p.W) {              // the mask words are fetched one word ahead
-          nx0 = row_word(p, it.h, it.u0, bw + 1, true);
-          nx1 = row_word(p, it.h, it.u0 + 1, bw + 1, it.has1);
-        }
+        if ((bw & 63) == 0 && (bw > 0 || p.W > 64)) rw.load(p, it, bw, lane);
+        bx0 = rw.row0(bw);
+        bx1 = rw.row1(bw);
         bx = bx0 | bx1;
       }
       const int bit = __ffs(bx) - 1;
@@ -415,6 +448,10 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
       cb = nb;
     }
     tc_commit_e(smem_u32(&ctl->q_empty));   // every S of this item has been issued
+    // No S can follow until the next item's Q tiles have arrived, and their load starts only now:
+    // issue the older parked PV at once (the younger one's P is still being computed; it goes out
+    // after the next item's bookkeeping, see above).
+    if (npend == 2) pop();
   }
   while (npend > 0) pop();
 #ifdef SA_TRACE
@@ -489,14 +526,16 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
                                          // of s_full[t][.] is consumed in order, none is skipped)
   int sched_n = 0;
 #ifdef SA_TRACE
-  uint32_t tr_acc[5] = {0, 0, 0, 0, 0}, tr_last = clock(), tr_n = 0;
+  uint32_t tr_acc[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, tr_last = clock(), tr_n = 0, tr_items = 0;
 #define SA_TR(i) { const uint32_t now_ = clock(); tr_acc[i] += now_ - tr_last; tr_last = now_; if (i == 4) ++tr_n; }
 #else
 #define SA_TR(i)
 #endif
   for (;;) {
     const int ss = sched_n % kSched;
+    SA_TR(0);
     mbar_wait(smem_u32(&ctl->sched_full[ss]), (sched_n / kSched) & 1, 20);
+    SA_TR(5);
     const int item = ctl->sched_item[ss];
     __syncwarp();
     if (lane == 0) mbar_arrive(smem_u32(&ctl->sched_empty[ss]));
@@ -512,7 +551,12 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     // scores, it becomes the row's softmax reference point for the whole item: no running max, no
     // rescale, and the row-max pass (a third of the softmax instructions) disappears. Otherwise the
     // warp keeps the exact running max. Either way the result is the same softmax.
+    RowWalk rw;
+    rw.load(p, it, 0, lane);
+    const float kmax2 = p.kmax2 ? __ldg(p.kmax2 + it.bh) : 0.f;   // in flight while Q arrives
+    SA_TR(0);
     mbar_wait(smem_u32(&ctl->q_full), qf_phase, 24);
+    SA_TR(6);
     qf_phase ^= 1u;
     float bound = 0.f;
     if (exists) {
@@ -532,26 +576,23 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
           qn2 = fmaf(hi, hi, qn2);
         }
       }
-      bound = p.kmax2 ? c * sqrtf(qn2) * sqrtf(__ldg(p.kmax2 + it.bh)) : INFINITY;   // no bound: exact max
+      bound = p.kmax2 ? c * sqrtf(qn2) * sqrtf(kmax2) : INFINITY;   // no bound: exact max
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(smem_u32(&ctl->q_empty));   // this warp is done with the Q tiles
+    SA_TR(7);
 
     float m_run = -INFINITY, l_run = 0.f;
     bool started = false;
     bool fixed = false;                  // warp-uniform: m_run is the bound, fixed for the item
     uint32_t prev_unit = 0xFFFFFFFEu;    // this tile's previous unit in the item
     // Walk this tile's own bit-row. A unit's number in the union walk order (which the MMA issuer
-    // follows) is the popcount of both rows below its bit. The mask words are fetched one word
-    // ahead and the next unit's bookkeeping is computed in the same straight-line block as the
-    // exponentials, so neither sits in the cycle S -> softmax -> PV -> next S.
-    uint32_t nx0 = row_word(p, it.h, it.u0, 0, true), nx1 = row_word(p, it.h, it.u0 + 1, 0, it.has1);
+    // follows) is the popcount of both rows below its bit. The next unit's bookkeeping is computed
+    // in the same straight-line block as the exponentials, so it does not sit in the cycle
+    // S -> softmax -> PV -> next S.
     for (int w = 0; w < p.W; ++w) {
-      const uint32_t x0 = nx0, x1 = nx1;
-      if (w + 1 < p.W) {
-        nx0 = row_word(p, it.h, it.u0, w + 1, true);
-        nx1 = row_word(p, it.h, it.u0 + 1, w + 1, it.has1);
-      }
+      if ((w & 63) == 0 && w > 0) rw.load(p, it, w, lane);
+      const uint32_t x0 = rw.row0(w), x1 = rw.row1(w);
       uint32_t xm = t == 0 ? x0 : x1;
       const uint32_t wbase = wg;
       wg += __popc(x0) + __popc(x1);
@@ -652,7 +693,9 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     const size_t grow = static_cast<size_t>(it.row0) + static_cast<size_t>(u) * kBlk + row;
     uint4* orow = reinterpret_cast<uint4*>(p.out + grow * kD);
     if (started) {
+      SA_TR(0);
       mbar_wait(smem_u32(&ctl->o_full[t]), o_phase, 22);
+      SA_TR(8);
       o_phase ^= 1u;
       tc_fence_after();
       const float inv = l_run > 0.f ? 1.f / l_run : 0.f;
@@ -661,20 +704,25 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
         uint32_t orr[32];
         tmem_ld32(tm_o + cc * 32, orr);
         tc_wait_ld();
+        // 32 columns -> 64 B of the row: two 256-bit stores, a full 32 B sector per lane each
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-          uint4 v;
-          v.x = pack_bf16x2(__uint_as_float(orr[8 * i + 0]) * inv, __uint_as_float(orr[8 * i + 1]) * inv);
-          v.y = pack_bf16x2(__uint_as_float(orr[8 * i + 2]) * inv, __uint_as_float(orr[8 * i + 3]) * inv);
-          v.z = pack_bf16x2(__uint_as_float(orr[8 * i + 4]) * inv, __uint_as_float(orr[8 * i + 5]) * inv);
-          v.w = pack_bf16x2(__uint_as_float(orr[8 * i + 6]) * inv, __uint_as_float(orr[8 * i + 7]) * inv);
-          orow[cc * 4 + i] = v;
+        for (int i = 0; i < 2; ++i) {
+          uint32_t v[8];
+#pragma unroll
+          for (int k = 0; k < 8; ++k)
+            v[k] = pack_bf16x2(__uint_as_float(orr[16 * i + 2 * k]) * inv,
+                               __uint_as_float(orr[16 * i + 2 * k + 1]) * inv);
+          st_global_256(orow + cc * 4 + i * 2, v);
         }
       }
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(smem_u32(&ctl->o_free[t]));
       p.lse[grow] = l_run > 0.f ? 0.6931471805599453f * (m_run + lg2(l_run)) : -INFINITY;
+      SA_TR(9);
+#ifdef SA_TRACE
+      ++tr_items;
+#endif
     } else {
       const uint4 z = make_uint4(0u, 0u, 0u, 0u);
 #pragma unroll
@@ -684,8 +732,9 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
   }
 #ifdef SA_TRACE
   if (lane == 0 && blockIdx.x < 2 && quarter == 0)
-    printf("trace cta %d wg %d blocks %u: other+epi %u | wait_s %u | ld %u | max+resc %u | exp+st %u (clk per block)\n",
-           blockIdx.x, t, tr_n, tr_acc[0] / tr_n, tr_acc[1] / tr_n, tr_acc[2] / tr_n, tr_acc[3] / tr_n, tr_acc[4] / tr_n);
+    printf("trace cta %d wg %d blocks %u: other %u | wait_s %u | ld %u | max+resc %u | exp+st %u (clk per block); items %u: sched %u | q_full %u | norms %u | o_full %u | epilogue %u (clk per item)\n",
+           blockIdx.x, t, tr_n, tr_acc[0] / tr_n, tr_acc[1] / tr_n, tr_acc[2] / tr_n, tr_acc[3] / tr_n, tr_acc[4] / tr_n,
+           tr_items, tr_acc[5] / tr_items, tr_acc[6] / tr_items, tr_acc[7] / tr_items, tr_acc[8] / tr_items, tr_acc[9] / tr_items);
 #endif
 }
 

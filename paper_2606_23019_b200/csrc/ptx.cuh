@@ -364,6 +364,12 @@ __device__ __forceinline__ void exp2_fma_pipe(uint64_t x, float& e0, float& e1) 
   e1 = __int_as_float(__float_as_int(q1) + (__float_as_int(r1) << 23));
 }
 
+// one 32 B sector per lane per instruction (sm_100: 256-bit global store)
+__device__ __forceinline__ void st_global_256(void* ptr, const uint32_t (&v)[8]) {
+  asm volatile("st.global.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"
+               ::"l"(ptr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7])
+               : "memory");
+}
 __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
   uint32_t r;
   asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
