@@ -409,6 +409,22 @@ def test_next1_262144_tokens_sampled_units(sa):
     _sampled_unit_parity(sa, cfg, q, k, v, bits, bits_t, variant=0, n_heads=2)
 
 
+def test_more_than_64_mask_words_sampled_units(sa):
+    # beyond the paper's longest sequence: 2112 key blocks = 66 mask words per row, so every role of the
+    # kernel reloads its 64-word window of the bit-rows once per item (K1); one head, 2% density
+    cfg = inputs.seq_grid_config(270336, H=1, n_valid=270336 - 5)
+    assert cfg.W == 66
+    q, k, v = inputs.make_qkv(cfg)
+    inputs.poison_padding(cfg, k, v)
+    scores, density = inputs.iid_block_scores(cfg, 0.02)
+    bits_t = sa.sa_pack_mask(torch.from_numpy(scores).cuda(), torch.from_numpy(density).cuda(),
+                             force_diag=True)
+    torch.cuda.synchronize()
+    bits = host_bits(bits_t)
+    assert (bits == oracle.pack_mask(scores, density, 1)).all()
+    _sampled_unit_parity(sa, cfg, q, k, v, bits, bits_t, variant=0, n_heads=1)
+
+
 @pytest.mark.parametrize("N", [1024, 4096])
 def test_next1_short_sequences_full_compare(sa, N):
     # the short end of the grid (8 and 32 key blocks: fewer work items than SMs), full compare
