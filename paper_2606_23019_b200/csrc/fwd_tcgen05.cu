@@ -699,25 +699,28 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
       o_phase ^= 1u;
       tc_fence_after();
       const float inv = l_run > 0.f ? 1.f / l_run : 0.f;
+      // the whole row of O to registers first (the S registers are dead here), O_t released to the
+      // next item's first PV before the conversion and the stores
+      uint32_t orr[4][32];
+#pragma unroll
+      for (int cc = 0; cc < 4; ++cc) tmem_ld32(tm_o + cc * 32, orr[cc]);
+      tc_wait_ld();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(smem_u32(&ctl->o_free[t]));
 #pragma unroll
       for (int cc = 0; cc < 4; ++cc) {
-        uint32_t orr[32];
-        tmem_ld32(tm_o + cc * 32, orr);
-        tc_wait_ld();
         // 32 columns -> 64 B of the row: two 256-bit stores, a full 32 B sector per lane each
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
           uint32_t v[8];
 #pragma unroll
           for (int k = 0; k < 8; ++k)
-            v[k] = pack_bf16x2(__uint_as_float(orr[16 * i + 2 * k]) * inv,
-                               __uint_as_float(orr[16 * i + 2 * k + 1]) * inv);
+            v[k] = pack_bf16x2(__uint_as_float(orr[cc][16 * i + 2 * k]) * inv,
+                               __uint_as_float(orr[cc][16 * i + 2 * k + 1]) * inv);
           st_global_256(orow + cc * 4 + i * 2, v);
         }
       }
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(smem_u32(&ctl->o_free[t]));
       p.lse[grow] = l_run > 0.f ? 0.6931471805599453f * (m_run + lg2(l_run)) : -INFINITY;
       SA_TR(9);
 #ifdef SA_TRACE
