@@ -54,23 +54,19 @@ constexpr float kRescaleThreshold = 8.0f; // log2 units
 constexpr float kBoundSlack = 64.0f;      // log2 units: how far the Cauchy-Schwarz bound may lie above
                                           // the first block's row maximum and still be used (2^-64 of
                                           // headroom is left before fp32 / bf16 flush to zero at 2^-126)
-// Tunables of the softmax (defaults chosen by measurement on B200, profiles/):
+// Tunable of the softmax (default chosen by measurement on B200):
 //  SA_POLY_PAIRS: of every 4 consecutive column pairs, how many take exp2 on the FMA pipe
 //  (Cody-Waite split + degree-3 polynomial) instead of MUFU.EX2 -- the MUFU pipe (16/clk/SM)
-//  would otherwise need as many cycles per tile as the two MMAs.
-//  SA_PCHUNKS: in how many pieces P is handed to the PV MMA (the MMA of the first keys starts
-//  while the exponentials of the later ones are still being computed).
+//  would otherwise need as many cycles per tile as the two MMAs. Off: under the power cap the
+//  extra instructions cost more than the shorter exponential phase gains.
 #ifndef SA_POLY_PAIRS
 #define SA_POLY_PAIRS 0
 #endif
-#ifndef SA_PCHUNKS
-#define SA_PCHUNKS 2
-#endif
 constexpr int kPolyPairs = SA_POLY_PAIRS;
-constexpr int kPChunks = SA_PCHUNKS;
 static_assert(kPolyPairs >= 0 && kPolyPairs <= 4, "SA_POLY_PAIRS in 0..4");
-static_assert(kPChunks == 1 || kPChunks == 2 || kPChunks == 4, "SA_PCHUNKS in {1,2,4}");
-static_assert(kPChunks == 2, "the MMA issuer takes P in two pieces");
+// P is handed to the PV MMA in two pieces of 64 keys (p_full[..][0], [1]): the MMAs of the first
+// keys start while the exponentials of the later ones are still being computed.
+constexpr int kPChunks = 2;
 
 // shared memory map (offsets from a 1024 B aligned base)
 constexpr uint32_t kOffQ = 0;                                   // 2 query tiles
