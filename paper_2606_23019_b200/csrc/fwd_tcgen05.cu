@@ -419,7 +419,9 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
         if (first[t]) ++n_started[t];
         first[t] = false;
         ++wg;
+        IT_TR(0);
         if (!k_ready) k_ready = mbar_try_wait(cb.k_full, cb.kphase);
+        IT_TR(2);
         if (npend == 2) pop();           // PV of the oldest unit: it frees this unit's S buffer
         if (!k_ready) {
           IT_TR(0);
@@ -527,7 +529,15 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
 #else
 #define SA_TR(i)
 #endif
-  for (;;) {
+  // Per item: what the walk needs (the item, its bit-rows, the rows' score bound). next_item() takes
+  // the next item from the scheduler ring and waits for its Q tiles; it is called for item n+1
+  // BEFORE the epilogue of item n, so that the wait for the Q tiles and the row norms fall into the
+  // time this warpgroup would otherwise spend waiting for the last PV of item n.
+  Item it{};
+  bool exists = false;
+  RowWalk rw;
+  float bound = 0.f;
+  auto next_item = [&]() {
     const int ss = sched_n % kSched;
     SA_TR(0);
     mbar_wait(smem_u32(&ctl->sched_full[ss]), (sched_n / kSched) & 1, 20);
@@ -536,10 +546,9 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     __syncwarp();
     if (lane == 0) mbar_arrive(smem_u32(&ctl->sched_empty[ss]));
     ++sched_n;
-    if (item < 0) break;
-    const Item it = decode_item(p, item, items_per_head);
-    const int u = it.u0 + t;
-    const bool exists = t == 0 || it.has1;   // tile 1 is empty in single-row items and past the last row
+    if (item < 0) return false;
+    it = decode_item(p, item, items_per_head);
+    exists = t == 0 || it.has1;   // tile 1 is empty in single-row items and past the last row
 
     // An upper bound of every score of this query row (Cauchy-Schwarz): scale * |q_i| * max_j |k_j|,
     // in the log2 domain. |q_i| comes from the Q tile in shared memory (128B-swizzled rows), max |k|
@@ -547,14 +556,13 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     // scores, it becomes the row's softmax reference point for the whole item: no running max, no
     // rescale, and the row-max pass (a third of the softmax instructions) disappears. Otherwise the
     // warp keeps the exact running max. Either way the result is the same softmax.
-    RowWalk rw;
     rw.load(p, it, 0, lane);
     const float kmax2 = p.kmax2 ? __ldg(p.kmax2 + it.bh) : 0.f;   // in flight while Q arrives
     SA_TR(0);
     mbar_wait(smem_u32(&ctl->q_full), qf_phase, 24);
     SA_TR(6);
     qf_phase ^= 1u;
-    float bound = 0.f;
+    bound = 0.f;
     if (exists) {
       const uint32_t qrow = smem_base + kOffQ + t * kTileBytes + row * 128;
       float qn2 = 0.f;
@@ -577,7 +585,11 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     __syncwarp();
     if (lane == 0) mbar_arrive(smem_u32(&ctl->q_empty));   // this warp is done with the Q tiles
     SA_TR(7);
+    return true;
+  };
 
+  bool have_item = next_item();
+  while (have_item) {
     float m_run = -INFINITY, l_run = 0.f;
     bool started = false;
     bool fixed = false;                  // warp-uniform: m_run is the bound, fixed for the item
@@ -684,10 +696,12 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
       }
     }
 
-    if (!exists) continue;
     // ---- epilogue: O / l -> bf16, lse = ln2 * (m + log2 l); empty row -> 0 / -inf
-    const size_t grow = static_cast<size_t>(it.row0) + static_cast<size_t>(u) * kBlk + row;
+    const bool wrote = exists;
+    const size_t grow = static_cast<size_t>(it.row0) + static_cast<size_t>(it.u0 + t) * kBlk + row;
     uint4* orow = reinterpret_cast<uint4*>(p.out + grow * kD);
+    have_item = next_item();             // (overwrites it, exists, rw, bound)
+    if (!wrote) continue;
     if (started) {
       SA_TR(0);
       mbar_wait(smem_u32(&ctl->o_full[t]), o_phase, 22);
