@@ -37,8 +37,8 @@ UNIT = "TFLOP/s"
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the attention kernel at the bench
 # workload, from the `ncu --set full` capture summarised in profiles/ (None until captured).
-NCU_TRAFFIC_BYTES = {"C4": 3265493776}   # dram__bytes_read.sum + dram__bytes_write.sum, one launch
-NCU_TRAFFIC_SOURCE = {"C4": "profiles/r1e_fwd_tcgen05_c4_full.md"}
+NCU_TRAFFIC_BYTES = {"C4": 3306511304}   # dram__bytes_read.sum + dram__bytes_write.sum, one launch
+NCU_TRAFFIC_SOURCE = {"C4": "profiles/r1f_fwd_tcgen05_c4_full.md"}
 
 
 # ------------------------------------------------------------------ pure helpers (CPU-testable)
