@@ -9,7 +9,8 @@
 // which are L2-resident: 56 MB at the 720p shape); keys > T are kept, and of the keys == T the
 // first r in flat-index order, r = k_h - #(keys > T). Index order needs a prefix count of the
 // ties: one per-row tie count pass, then each row's warp sums the rows before it and walks its
-// own row 32 key blocks at a time with __ballot_sync, which is also what packs the bits.
+// own row 32 key blocks at a time with __ballot_sync, which is also what packs the bits. When all
+// keys equal to T are kept (T unique: the usual case) both the tie counts and the prefix are skipped.
 // Bandwidth/ALU work only; no tensor cores (HBM/L2-bound streaming, coalesced 128 B per warp).
 #include "common.cuh"
 
@@ -22,6 +23,7 @@ constexpr int kHistRowsPerBlock = 16;     // rows of one head per histogram bloc
 struct HeadState {      // per head, per pass p = 0..3: state after resolving passes < p
   uint32_t prefix[5];   // high bits fixed so far (prefix[p] has the top 8*p bits set)
   uint32_t k_rem[5];    // how many keys with that prefix (ranked from the largest) still to take
+  uint32_t n_equal;     // after the last pass: how many keys equal T = prefix[4] the head holds
 };
 
 // workspace: hist uint32 [H][4][256] | HeadState [H] | row_ties uint32 [H][NQB]
@@ -71,7 +73,7 @@ __device__ __forceinline__ uint32_t keep_count(float density, int NQB, int NKB, 
 // result lands in shared memory, and block 0 of the head records it for later kernels.
 __device__ void resolve(int pass, int h, const float* density, int NQB, int NKB, int force_diag,
                         const uint32_t* hist, HeadState* state, uint32_t* s_prefix,
-                        uint32_t* s_krem, bool record) {
+                        uint32_t* s_krem, bool record, uint32_t* s_nequal = nullptr) {
   __shared__ uint32_t s_suffix[256];
   if (pass == 0) {
     if (threadIdx.x == 0) {
@@ -122,7 +124,12 @@ __device__ void resolve(int pass, int h, const float* density, int NQB, int NKB,
       const int shift = 32 - 8 * pass;
       *s_prefix = prev_prefix | (static_cast<uint32_t>(bin) << shift);
       *s_krem = prev_krem - above;
-      if (record) { state[h].prefix[pass] = *s_prefix; state[h].k_rem[pass] = *s_krem; }
+      if (record) {
+        state[h].prefix[pass] = *s_prefix;
+        state[h].k_rem[pass] = *s_krem;
+        if (pass == 4) state[h].n_equal = s_suffix[bin];   // the bin of the full key
+      }
+      if (s_nequal) *s_nequal = s_suffix[bin];
     }
   }
   __syncthreads();
@@ -191,10 +198,13 @@ __global__ void __launch_bounds__(256)
 pack_row_ties_kernel(const float* __restrict__ scores, const float* __restrict__ density, int NQB,
                      int NKB, int force_diag, const uint32_t* __restrict__ hist, HeadState* state,
                      uint32_t* __restrict__ row_ties) {
-  __shared__ uint32_t s_T, s_r;
+  __shared__ uint32_t s_T, s_r, s_neq;
   const int h = blockIdx.y;
-  resolve(4, h, density, NQB, NKB, force_diag, hist, state, &s_T, &s_r, blockIdx.x == 0);
+  resolve(4, h, density, NQB, NKB, force_diag, hist, state, &s_T, &s_r, blockIdx.x == 0, &s_neq);
   const uint32_t T = s_T;
+  // every key equal to T is kept (always so when T is unique, the usual case for real-valued
+  // scores): their order does not matter and nobody reads the per-row counts
+  if (s_r == s_neq) return;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int u = blockIdx.x * 8 + warp;
   if (u >= NQB) return;
@@ -217,22 +227,40 @@ pack_write_kernel(const float* __restrict__ scores, int NQB, int NKB, int W, int
   if (u >= NQB) return;
   const uint32_t T = state[h].prefix[4];
   const uint32_t r = state[h].k_rem[4];
+  const bool all_equal_kept = r == state[h].n_equal;     // then keep = key >= T, no tie order needed
   uint32_t before = 0;
-  for (int j = lane; j < u; j += 32) before += __ldg(row_ties + static_cast<size_t>(h) * NQB + j);
-  for (int o = 16; o; o >>= 1) before += __shfl_xor_sync(0xFFFFFFFFu, before, o);
+  if (!all_equal_kept) {
+    for (int j = lane; j < u; j += 32) before += __ldg(row_ties + static_cast<size_t>(h) * NQB + j);
+    for (int o = 16; o; o >>= 1) before += __shfl_xor_sync(0xFFFFFFFFu, before, o);
+  }
   const float* row = scores + (static_cast<size_t>(h) * NQB + u) * NKB;
   uint32_t* out = mask_bits + (static_cast<size_t>(h) * NQB + u) * W;
-  for (int w = 0; w < W; ++w) {
-    const int v = w * 32 + lane;
-    uint32_t key = 0u;
-    const bool valid = v < NKB;
-    if (valid) key = score_key(__ldg(row + v), force_diag && u == v);
-    const uint32_t gt = __ballot_sync(0xFFFFFFFFu, valid && key > T);
-    const uint32_t eq = __ballot_sync(0xFFFFFFFFu, valid && key == T);
-    const uint32_t my_rank = before + __popc(eq & ((1u << lane) - 1u));
-    const uint32_t eq_keep = __ballot_sync(0xFFFFFFFFu, valid && key == T && my_rank < r);
-    if (lane == 0) out[w] = gt | eq_keep;
-    before += __popc(eq);
+  for (int w0 = 0; w0 < W; w0 += 4) {                     // four loads in flight per lane (L2 latency)
+    float x[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const int v = (w0 + q) * 32 + lane;
+      x[q] = v < NKB ? __ldg(row + v) : 0.f;
+    }
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const int w = w0 + q;
+      if (w >= W) break;
+      const int v = w * 32 + lane;
+      const bool valid = v < NKB;
+      const uint32_t key = valid ? score_key(x[q], force_diag && u == v) : 0u;
+      uint32_t bits;
+      if (all_equal_kept) {
+        bits = __ballot_sync(0xFFFFFFFFu, valid && key >= T);
+      } else {
+        const uint32_t gt = __ballot_sync(0xFFFFFFFFu, valid && key > T);
+        const uint32_t eq = __ballot_sync(0xFFFFFFFFu, valid && key == T);
+        const uint32_t my_rank = before + __popc(eq & ((1u << lane) - 1u));
+        bits = gt | __ballot_sync(0xFFFFFFFFu, valid && key == T && my_rank < r);
+        before += __popc(eq);
+      }
+      if (lane == 0) out[w] = bits;
+    }
   }
 }
 
