@@ -409,6 +409,34 @@ def test_next1_262144_tokens_sampled_units(sa):
     _sampled_unit_parity(sa, cfg, q, k, v, bits, bits_t, variant=0, n_heads=2)
 
 
+def test_forward_call_is_cuda_graph_capturable(sa):
+    # the forward call (schedule pre-pass + attention kernel, tensor maps passed by value) only
+    # enqueues work on the caller's stream: a captured graph replays to the same bits
+    cfg = inputs.seq_grid_config(4096, H=3, seed=7)
+    q, k, v = [x.cuda() for x in inputs.make_qkv(cfg)]
+    scores, density = inputs.iid_block_scores(cfg, 0.25)
+    bits_t = sa.sa_pack_mask(torch.from_numpy(scores).cuda(), torch.from_numpy(density).cuda(),
+                             force_diag=True)
+    ws = torch.empty(sa.sa_fwd_workspace_bytes(cfg.B, cfg.H, cfg.N, cfg.Bq), dtype=torch.uint8,
+                     device="cuda")
+    ref_o, ref_l = sa.sa_block_sparse_attn_fwd_ex(q, k, v, bits_t, cfg.Bq, cfg.Bk, cfg.scale,
+                                                  n_valid=cfg.n_valid, workspace=ws)
+    torch.cuda.synchronize()
+    out = torch.zeros_like(ref_o)
+    lse = torch.zeros_like(ref_l)
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=stream):
+            sa.sa_block_sparse_attn_fwd_ex(q, k, v, bits_t, cfg.Bq, cfg.Bk, cfg.scale,
+                                           n_valid=cfg.n_valid, out=out, lse=lse, workspace=ws)
+        for _ in range(2):
+            out.zero_()
+            graph.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(out, ref_o) and torch.equal(lse, ref_l)
+
+
 def test_more_than_64_mask_words_sampled_units(sa):
     # beyond the paper's longest sequence: 2112 key blocks = 66 mask words per row, so every role of the
     # kernel reloads its 64-word window of the bit-rows once per item (K1); one head, 2% density
