@@ -142,7 +142,7 @@ SA_API sa_status sa_fidelity_from_lse(const float* lse_dense, const float* lse_s
  *   lse[b,h,i]   = ln sum_j exp(scale * <q_i, k_j>)                       (natural log)
  * with j ranging over the tokens of the key blocks whose bit is set in row (h, i / Bq). Masked key
  * blocks are never loaded and never multiplied. A row with no active key gives out = 0, lse = -inf.
- *   q, k, v, out : bf16 [B][H][N][D] contiguous, 16 B aligned (out: 32 B when D = 128);  lse : fp32 [B][H][N]
+ *   q, k, v, out : bf16 [B][H][N][D] contiguous, 16 B aligned;  lse : fp32 [B][H][N]
  *   scale        : softmax scale (e.g. 1/sqrt(D)); arithmetic is bf16 x bf16 -> fp32.
  * All N tokens are real. Uses an internal workspace (grown with cudaMalloc on first use / when a
  * larger problem arrives, which synchronises; freed at process exit). */

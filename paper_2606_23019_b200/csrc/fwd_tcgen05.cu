@@ -518,6 +518,7 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
   const uint32_t lane_base = static_cast<uint32_t>(quarter * 32) << 16;
   const uint32_t tm_o = tmem + lane_base + 256 + t * 128;
   const float c = p.scale_log2;
+  const bool out32 = (reinterpret_cast<uintptr_t>(p.out) & 31u) == 0;   // rows are 256 B apart
   uint32_t o_phase = 0, qf_phase = 0;
   uint32_t wg = 0;                       // global unit counter, in step with the MMA issuer
   uint32_t nmine = 0;                    // this tile's units so far (barrier selection: every phase
@@ -721,6 +722,7 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
 #pragma unroll
       for (int cc = 0; cc < 4; ++cc) {
         // 32 columns -> 64 B of the row: two 256-bit stores, a full 32 B sector per lane each
+        // (four 128-bit stores if the caller's out is only 16 B aligned, which the ABI allows)
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
           uint32_t v[8];
@@ -728,7 +730,12 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
           for (int k = 0; k < 8; ++k)
             v[k] = pack_bf16x2(__uint_as_float(orr[cc][16 * i + 2 * k]) * inv,
                                __uint_as_float(orr[cc][16 * i + 2 * k + 1]) * inv);
-          st_global_256(orow + cc * 4 + i * 2, v);
+          if (out32) {
+            st_global_256(orow + cc * 4 + i * 2, v);
+          } else {
+            orow[cc * 4 + i * 2] = make_uint4(v[0], v[1], v[2], v[3]);
+            orow[cc * 4 + i * 2 + 1] = make_uint4(v[4], v[5], v[6], v[7]);
+          }
         }
       }
       p.lse[grow] = l_run > 0.f ? 0.6931471805599453f * (m_run + lg2(l_run)) : -INFINITY;

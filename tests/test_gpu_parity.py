@@ -409,6 +409,26 @@ def test_next1_262144_tokens_sampled_units(sa):
     _sampled_unit_parity(sa, cfg, q, k, v, bits, bits_t, variant=0, n_heads=2)
 
 
+def test_out_aligned_to_16_bytes_only(sa):
+    # the ABI asks for 16-byte alignment; the 128-shape kernel writes rows with 256-bit stores only
+    # when out is 32-byte aligned and with 128-bit stores otherwise: same bits either way
+    cfg = inputs.seq_grid_config(2048, H=2, seed=11)
+    q, k, v = [x.cuda() for x in inputs.make_qkv(cfg)]
+    scores, density = inputs.iid_block_scores(cfg, 0.5)
+    bits_t = sa.sa_pack_mask(torch.from_numpy(scores).cuda(), torch.from_numpy(density).cuda(),
+                             force_diag=True)
+    ref_o, ref_l = sa.sa_block_sparse_attn_fwd_ex(q, k, v, bits_t, cfg.Bq, cfg.Bk, cfg.scale,
+                                                  n_valid=cfg.n_valid)
+    buf = torch.zeros(q.numel() + 8, dtype=torch.bfloat16, device="cuda")
+    out = buf[8:].view_as(q)                      # 16 bytes past an aligned base
+    assert out.data_ptr() % 32 == 16
+    out, lse = sa.sa_block_sparse_attn_fwd_ex(q, k, v, bits_t, cfg.Bq, cfg.Bk, cfg.scale,
+                                              n_valid=cfg.n_valid, out=out)
+    torch.cuda.synchronize()
+    assert torch.equal(out, ref_o) and torch.equal(lse, ref_l)
+    assert (buf[:8] == 0).all()
+
+
 def test_forward_call_is_cuda_graph_capturable(sa):
     # the forward call (schedule pre-pass + attention kernel, tensor maps passed by value) only
     # enqueues work on the caller's stream: a captured graph replays to the same bits
