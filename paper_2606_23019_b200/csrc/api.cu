@@ -1,5 +1,6 @@
 // api.cu -- the C ABI of libscalingattn.so (include/scalingattn.h): argument validation, error
 // reporting, workspace carving and kernel dispatch. No arithmetic of the method lives here.
+#include <atomic>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
@@ -12,7 +13,7 @@ namespace {
 
 thread_local char g_err[512] = "";
 thread_local int g_last_launches = 0;
-int g_variant = 0;
+std::atomic<int> g_variant{0};   // debug hook (sa_set_fwd_variant): read once per call
 
 sa_status fail(sa_status s, const char* fmt, ...) {
   va_list ap;
@@ -297,20 +298,25 @@ static sa_status fwd_ex_impl(const void* q, const void* k, const void* v, const 
   p.scale = scale;
   p.scale_log2 = scale * 1.4426950408889634f;
   const sa::FwdWorkspace w = sa::carve_fwd_workspace(workspace, B, H, p.NQB);
-  p.unit_order = w.unit_order;
+  p.items = w.items;
+  p.n_items_dev = w.n_items;
   p.counter = w.cursor;
-  const bool fast = (g_variant != 1 && D == 128);
+  const int variant = g_variant.load(std::memory_order_relaxed);
+  const bool fast = (variant != 1 && D == 128);
   // the per-row score bound saves ~6% of the attention kernel but costs one more (~8 us) launch:
   // not worth it on problems of a few thousand tiles, which then keep the exact running max
   const bool big = static_cast<long long>(B) * H * p.NQB * p.NKB >= 16384;
-  p.kmax2 = (fast && (g_variant == 2 || (g_variant == 0 && big))) ? w.kmax2 : nullptr;
+  p.kmax2 = (fast && (variant == 2 || (variant == 0 && big))) ? w.kmax2 : nullptr;
   // The tcgen05 kernel works on PAIRS of query blocks (shared K/V tiles). When there are fewer pairs
   // than two waves of CTAs (short sequences) single-row items fill the SMs better.
+  int n_sm = 0;
+  cudaError_t e = sa::device_sm_count(&n_sm);
+  if (e != cudaSuccess) return cuda_fail(e, "device query");
   const long long n_pairs = static_cast<long long>(B) * H * ((p.NQB + 1) / 2);
-  const int rows_per_item = (fast && (g_variant == 2 || (g_variant == 0 && n_pairs >= 2 * 148))) ? 2 : 1;
+  const int rows_per_item = (fast && (variant == 2 || (variant == 0 && n_pairs >= 2 * n_sm))) ? 2 : 1;
   p.rows_per_item = rows_per_item;
   p.n_items = B * H * ((p.NQB + rows_per_item - 1) / rows_per_item);
-  cudaError_t e = sa::launch_schedule(p, w, rows_per_item, st, &g_last_launches, reuse_schedule);
+  e = sa::launch_schedule(p, w, rows_per_item, st, &g_last_launches, reuse_schedule);
   if (e != cudaSuccess) return cuda_fail(e, "schedule pre-pass launch");
   cudaEvent_t ev_stop = nullptr;
   {
@@ -573,10 +579,10 @@ sa_status sa_enumerate_active_blocks(const uint32_t* mask_bits, int H, int NQB, 
 sa_status sa_set_fwd_variant(int variant) {
   if (variant < 0 || variant > 3)
     return fail(SA_ERR_INVALID_ARG, "sa_set_fwd_variant: variant %d not in {0,1,2,3}", variant);
-  g_variant = variant;
+  g_variant.store(variant, std::memory_order_relaxed);
   return SA_OK;
 }
-int sa_get_fwd_variant(void) { return g_variant; }
+int sa_get_fwd_variant(void) { return g_variant.load(std::memory_order_relaxed); }
 int sa_last_launch_count(void) { return g_last_launches; }
 
 const char* sa_status_string(sa_status s) {

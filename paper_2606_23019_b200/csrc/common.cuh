@@ -59,30 +59,41 @@ struct FwdParams {
   float scale;
   float scale_log2;   // scale * log2(e)
   // schedule (workspace)
-  const int32_t* unit_order;  // [n_items] item ids in issue order
+  const int2* items;          // work items in issue order: x = b*H + h, y = ua | ub << 16 (query blocks
+                              // of the item; ub = 0xFFFF: single-row item)
+  const int32_t* n_items_dev; // number of work items, written by the pre-pass (pair items: mask-dependent)
   int32_t* counter;           // dynamic scheduler cursor (zeroed by the pre-pass)
   const float* kmax2;         // [B*H] max |k|^2 over the valid keys (tcgen05 kernel only)
-  int n_items;
+  int n_items;                // host-side count: exact for single-row items, an upper bound for pairs
   int rows_per_item;          // query blocks per work item: 2 (a pair shares its K/V tiles) or 1
 };
 
-// Workspace layout for the forward pass (all int32):
+// Workspace layout for the forward pass (int32 words):
 //   [0]                  scheduler cursor
-//   [16 .. 16+BH)        per-(b,h) total cost
-//   [.. + BH)            (b,h) issue order (heaviest first)
+//   [1]                  number of work items
+//   [16 .. 16+BH)        per-(b,h) total cost (active tiles)
+//   [.. + BH)            per-(b,h) number of items
 //   [.. + BH)            fp32: per (b,h) max over the valid keys of |k|^2
-//   [.. + BH*items]      per-(b,h) item order (cost descending), local item index
-//   [.. + BH*items]      flattened issue order of global item ids
+//   int2 [BH*NQB]        per-(b,h) items, cost descending: {cost, ua | ub << 16}
+//   int2 [BH*NQB]        all items in issue order: {b*H + h, ua | ub << 16}
 struct FwdWorkspace {
   int32_t* cursor;
+  int32_t* n_items;
   int32_t* head_cost;
-  int32_t* head_order;
+  int32_t* head_count;
   float* kmax2;               // [B*H] max over valid keys of |k|^2
-  int32_t* local_order;
-  int32_t* unit_order;
+  int2* local_items;
+  int2* items;
 };
 size_t fwd_workspace_bytes(int B, int H, int NQB);
 FwdWorkspace carve_fwd_workspace(void* ws, int B, int H, int NQB);
+
+// per-device state (device.cu): SM count of the current device; dynamic shared-memory opt-in of a
+// kernel, set once per (device, kernel)
+enum SmemKernel { kSmemFwdTcgen05 = 0, kSmemSigTcgen05, kSmemScheduleItems, kSmemFwdMmaSync64,
+                  kSmemFwdMmaSync128, kNumSmemKernels };
+cudaError_t device_sm_count(int* n_sm);
+cudaError_t ensure_dynamic_smem(SmemKernel id, const void* func, int bytes);
 
 // launchers (each returns the cudaError_t of its launches; *n_launch += kernels enqueued)
 cudaError_t launch_schedule(const FwdParams& p, const FwdWorkspace& w, int rows_per_item,

@@ -88,8 +88,8 @@ __global__ void __launch_bounds__(BLK * 2, 1) fwd_mma_sync_kernel(const FwdParam
   const uint32_t sK0 = sQ + TILE_BYTES;            // K[2]
   const uint32_t sV0 = sK0 + 2 * TILE_BYTES;       // V[2]
 
-  const int item = p.unit_order[blockIdx.x];
-  const int bh = item / p.NQB, u = item % p.NQB;
+  const int2 item = p.items[blockIdx.x];       // single-row items: x = b*H + h, y = query block | 0xFFFF << 16
+  const int bh = item.x, u = item.y & 0xFFFF;
   const int h = bh % p.H;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int g = lane >> 2, t = lane & 3;
@@ -253,8 +253,9 @@ __global__ void __launch_bounds__(BLK * 2, 1) fwd_mma_sync_kernel(const FwdParam
 template <int BLK, int D>
 cudaError_t launch(const FwdParams& p, cudaStream_t st) {
   constexpr size_t smem = 5ull * BLK * D * 2;
-  cudaError_t e = cudaFuncSetAttribute(fwd_mma_sync_kernel<BLK, D>,
-                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaError_t e = ensure_dynamic_smem(BLK == 64 ? kSmemFwdMmaSync64 : kSmemFwdMmaSync128,
+                                      reinterpret_cast<const void*>(fwd_mma_sync_kernel<BLK, D>),
+                                      static_cast<int>(smem));
   if (e != cudaSuccess) return e;
   fwd_mma_sync_kernel<BLK, D><<<p.n_items, BLK * 2, smem, st>>>(p);
   return cudaGetLastError();

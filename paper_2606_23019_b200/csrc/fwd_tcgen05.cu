@@ -78,7 +78,7 @@ struct __align__(8) Ctl {
   uint64_t s_full[2][2], p_full[2][2][4], pv_done[2][2];   // [tile][tile-local unit & 1]
   uint64_t o_full[2], o_free[2];
   uint64_t sched_full[kSched], sched_empty[kSched];
-  int32_t sched_item[kSched];
+  int2 sched_item[kSched];            // item record (x = -1: no more work)
   uint32_t tmem_base;
 };
 constexpr uint32_t kSmemBytes = kOffCtl + sizeof(Ctl) + 1024;   // + alignment slack
@@ -102,17 +102,21 @@ constexpr uint32_t kIdescQK = (1u << 4) | (1u << 7) | (1u << 10) | ((128u >> 3) 
                               ((128u >> 4) << 24);
 constexpr uint32_t kIdescPV = kIdescQK | (1u << 16);
 
+// A work item: query blocks ua (tile 0) and ub (tile 1) of one (batch, head); the schedule pre-pass
+// chooses the pairs (schedule.cu). Single-row items leave tile 1 empty.
 struct Item {
-  int bh, h, u0;
+  int bh, h, ua, ub;
   bool has1;
   int row0;            // first token row of the (b,h) slab in the [B*H*N][D] view
 };
-__device__ __forceinline__ Item decode_item(const FwdParams& p, int item, int items_per_head) {
+// item record: x = b*H + h (-1: no more work), y = ua | ub << 16 (ub = 0xFFFF: no second row)
+__device__ __forceinline__ Item decode_item(const FwdParams& p, int2 rec) {
   Item it;
-  it.bh = item / items_per_head;
+  it.bh = rec.x;
   it.h = it.bh % p.H;
-  it.u0 = p.rows_per_item * (item % items_per_head);
-  it.has1 = p.rows_per_item == 2 && it.u0 + 1 < p.NQB;   // single-row items leave tile 1 empty
+  it.ua = rec.y & 0xFFFF;
+  it.ub = (rec.y >> 16) & 0xFFFF;
+  it.has1 = it.ub != 0xFFFF;
   it.row0 = it.bh * p.N;
   return it;
 }
@@ -134,10 +138,10 @@ struct RowWalk {
   uint32_t a0 = 0, a1 = 0, b0 = 0, b1 = 0;
   __device__ __forceinline__ void load(const FwdParams& p, const Item& it, int base, int lane) {
     const int w0 = base + lane, w1 = base + 32 + lane;
-    a0 = w0 < p.W ? row_word(p, it.h, it.u0, w0, true) : 0u;
-    a1 = w1 < p.W ? row_word(p, it.h, it.u0, w1, true) : 0u;
-    b0 = w0 < p.W ? row_word(p, it.h, it.u0 + 1, w0, it.has1) : 0u;
-    b1 = w1 < p.W ? row_word(p, it.h, it.u0 + 1, w1, it.has1) : 0u;
+    a0 = w0 < p.W ? row_word(p, it.h, it.ua, w0, true) : 0u;
+    a1 = w1 < p.W ? row_word(p, it.h, it.ua, w1, true) : 0u;
+    b0 = w0 < p.W ? row_word(p, it.h, it.ub, w0, it.has1) : 0u;
+    b1 = w1 < p.W ? row_word(p, it.h, it.ub, w1, it.has1) : 0u;
   }
   // number of set bits of each row within the loaded 64 words
   __device__ __forceinline__ void counts(uint32_t& n0, uint32_t& n1) const {
@@ -163,8 +167,7 @@ struct Ring {
 // ------------------------------------------------------------------ warp 0: scheduler + TMA
 // Runs on every lane of warp 0 (converged); elect.sync inside the _e wrappers picks the issuer.
 __device__ void producer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, const CUtensorMap* tm_q,
-                         const CUtensorMap* tm_k, const CUtensorMap* tm_v, int items_per_head,
-                         int lane) {
+                         const CUtensorMap* tm_k, const CUtensorMap* tm_v, int lane) {
   Ring ring;
   uint32_t q_phase = 0;
   int sched_n = 0;
@@ -173,11 +176,12 @@ __device__ void producer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, const
   // item nobody waits for the atomic and the list lookup (two dependent global round trips, ~3 us
   // of idle tensor pipe per item otherwise). The list is longest-first inside a head, so the items
   // claimed early near the end are the light ones and the tail stays short.
+  const int n_items = __ldg(p.n_items_dev);
   auto claim_and_publish = [&]() {
     int idx = 0;
     if (lane == 0) idx = atomicAdd(p.counter, 1);
     idx = __shfl_sync(0xFFFFFFFFu, idx, 0);
-    const int it_id = idx < p.n_items ? __ldg(p.unit_order + idx) : -1;
+    const int2 it_id = idx < n_items ? __ldg(p.items + idx) : make_int2(-1, 0);
     const int ss = sched_n % kSched;
     mbar_wait(smem_u32(&ctl->sched_empty[ss]), ((sched_n / kSched) & 1) ^ 1u, 1);
     if (lane == 0) {
@@ -188,11 +192,11 @@ __device__ void producer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, const
     ++sched_n;
     return it_id;
   };
-  int next_item = claim_and_publish();
+  int2 next_item = claim_and_publish();
   for (;;) {
-    const int item = next_item;
-    if (item < 0) break;
-    const Item it = decode_item(p, item, items_per_head);
+    const int2 item = next_item;
+    if (item.x < 0) break;
+    const Item it = decode_item(p, item);
     // ... unless this item is a long one (a held-back item would then wait that long while another
     // CTA may be idle): long items claim their successor only when their own loads are out
     RowWalk rw;
@@ -211,7 +215,7 @@ __device__ void producer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, const
     mbar_expect_tx_e(qf, it.has1 ? 2 * kTileBytes : kTileBytes);
     for (int t = 0; t < (it.has1 ? 2 : 1); ++t) {
       const uint32_t dst = smem_base + kOffQ + t * kTileBytes;
-      const int y = it.row0 + (it.u0 + t) * kBlk;
+      const int y = it.row0 + (t == 0 ? it.ua : it.ub) * kBlk;
       tma_load_2d_e(dst, tm_q, 0, y, qf);
       tma_load_2d_e(dst + kHalfBytes, tm_q, 64, y, qf);
     }
@@ -275,7 +279,7 @@ struct Pend {
 // unit w-1 overlaps both. P(w-2) aliases S buffer (w & 1), so S(w) must follow PV(w-2) in the
 // (in-order) tensor pipe, which this order guarantees.
 __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uint32_t tmem,
-                           int items_per_head, int lane) {
+                           int lane) {
   Ring ring;
   uint32_t q_phase = 0, n_started[2] = {0, 0};
   uint32_t wg = 0;                       // global unit counter
@@ -320,12 +324,14 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     mbar_wait(smem_u32(&ctl->sched_full[ss]), (sched_n / kSched) & 1, 10);
     IT_TR(4);
     // warp-uniform by construction; the reduction tells the compiler so (see uni())
-    const int item = static_cast<int>(uni(static_cast<uint32_t>(ctl->sched_item[ss])));
+    int2 item;
+    item.x = static_cast<int>(uni(static_cast<uint32_t>(ctl->sched_item[ss].x)));
+    item.y = static_cast<int>(uni(static_cast<uint32_t>(ctl->sched_item[ss].y)));
     __syncwarp();
     if (lane == 0) mbar_arrive(smem_u32(&ctl->sched_empty[ss]));
     ++sched_n;
-    if (item < 0) break;
-    const Item it = decode_item(p, item, items_per_head);
+    if (item.x < 0) break;
+    const Item it = decode_item(p, item);
 
     RowWalk rw;
     uint32_t rem[2] = {0, 0};            // units each tile still has in this item
@@ -513,7 +519,7 @@ __device__ __forceinline__ float exp_tile(const uint32_t (&sr)[4][32], float c, 
 // One thread per query row: thread (quarter, lane) of warpgroup t owns TMEM lane 32*quarter+lane
 // of S_t / O_t, so row max and row sum need no shuffles.
 __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uint32_t tmem, int t,
-                           int quarter, int lane, int items_per_head) {
+                           int quarter, int lane) {
   const int row = quarter * 32 + lane;
   const uint32_t lane_base = static_cast<uint32_t>(quarter * 32) << 16;
   const uint32_t tm_o = tmem + lane_base + 256 + t * 128;
@@ -543,12 +549,12 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     SA_TR(0);
     mbar_wait(smem_u32(&ctl->sched_full[ss]), (sched_n / kSched) & 1, 20);
     SA_TR(5);
-    const int item = ctl->sched_item[ss];
+    const int2 item = ctl->sched_item[ss];
     __syncwarp();
     if (lane == 0) mbar_arrive(smem_u32(&ctl->sched_empty[ss]));
     ++sched_n;
-    if (item < 0) return false;
-    it = decode_item(p, item, items_per_head);
+    if (item.x < 0) return false;
+    it = decode_item(p, item);
     exists = t == 0 || it.has1;   // tile 1 is empty in single-row items and past the last row
 
     // An upper bound of every score of this query row (Cauchy-Schwarz): scale * |q_i| * max_j |k_j|,
@@ -699,7 +705,7 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
 
     // ---- epilogue: O / l -> bf16, lse = ln2 * (m + log2 l); empty row -> 0 / -inf
     const bool wrote = exists;
-    const size_t grow = static_cast<size_t>(it.row0) + static_cast<size_t>(it.u0 + t) * kBlk + row;
+    const size_t grow = static_cast<size_t>(it.row0) + static_cast<size_t>(t == 0 ? it.ua : it.ub) * kBlk + row;
     uint4* orow = reinterpret_cast<uint4*>(p.out + grow * kD);
     have_item = next_item();             // (overwrites it, exists, rw, bound)
     if (!wrote) continue;
@@ -768,7 +774,6 @@ fwd_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
   Ctl* ctl = reinterpret_cast<Ctl*>(smem_raw + (smem_base - raw) + kOffCtl);
   // warp index through a shuffle: the compiler then knows it is warp-uniform, and so is the role branch
   const int warp = __shfl_sync(0xFFFFFFFFu, static_cast<int>(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
-  const int items_per_head = (p.NQB + p.rows_per_item - 1) / p.rows_per_item;
 
   if (threadIdx.x == 0) {
     prefetch_tensormap(&tm_q);
@@ -808,13 +813,13 @@ fwd_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
   if (warp < 4) {
     setmaxnreg_dec<88>();
     if (warp == 0) {
-      producer(p, ctl, smem_base, &tm_q, &tm_k, &tm_v, items_per_head, lane);
+      producer(p, ctl, smem_base, &tm_q, &tm_k, &tm_v, lane);
     } else if (warp == 1) {
-      mma_issuer(p, ctl, smem_base, tmem, items_per_head, lane);
+      mma_issuer(p, ctl, smem_base, tmem, lane);
     }
   } else {
     setmaxnreg_inc<208>();
-    softmax_wg(p, ctl, smem_base, tmem, warp >= 8 ? 1 : 0, warp & 3, lane, items_per_head);
+    softmax_wg(p, ctl, smem_base, tmem, warp >= 8 ? 1 : 0, warp & 3, lane);
   }
   tc_fence_before();
   __syncthreads();
@@ -861,26 +866,19 @@ bool make_tile_map_128x64(void* map, const void* base, uint64_t rows) {
 
 cudaError_t launch_fwd_tcgen05(const FwdParams& p, void*, cudaStream_t st, int* n_launch,
                                const char** err_text) {
-  static int n_sm = 0;
-  static bool attr_set = false;
-  if (!attr_set) {
-    int dev = 0;
-    cudaError_t e = cudaGetDevice(&dev);
-    if (e != cudaSuccess) return e;
-    e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(fwd_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             static_cast<int>(kSmemBytes));
-    if (e != cudaSuccess) { *err_text = "cudaFuncSetAttribute(fwd_tcgen05_kernel)"; return e; }
-    attr_set = true;
-  }
+  int n_sm = 0;
+  cudaError_t e = device_sm_count(&n_sm);
+  if (e != cudaSuccess) return e;
+  e = ensure_dynamic_smem(kSmemFwdTcgen05, reinterpret_cast<const void*>(fwd_tcgen05_kernel),
+                          static_cast<int>(kSmemBytes));
+  if (e != cudaSuccess) { *err_text = "cudaFuncSetAttribute(fwd_tcgen05_kernel)"; return e; }
   CUtensorMap tq, tk, tv;
   const uint64_t rows = static_cast<uint64_t>(p.B) * p.H * p.N;
   if (!make_map(&tq, p.q, rows) || !make_map(&tk, p.k, rows) || !make_map(&tv, p.v, rows)) {
     *err_text = "cuTensorMapEncodeTiled failed";
     return cudaErrorInvalidValue;
   }
-  const int grid = p.n_items < n_sm ? p.n_items : n_sm;
+  const int grid = p.n_items < n_sm ? p.n_items : n_sm;   // n_items: upper bound (pairs are mask-dependent)
   fwd_tcgen05_kernel<<<grid, kThreads, kSmemBytes, st>>>(tq, tk, tv, p);
   *n_launch += 1;
   return cudaGetLastError();

@@ -3,18 +3,28 @@
 // One unit of work is (batch, head, query block) (the CRM iterator replaces the
 // dense KV-block iterator of FlashAttention, whose forward pass gives one thread block one query
 // block). The paper is silent on load balance; per-row popcounts are uneven (edge blocks, sinks,
-// per-head density), so the pre-pass orders the work: (b,h) groups heaviest first (keeps the
-// concurrently running CTAs on one or two heads, whose K/V then stay in L2) and, inside a group,
-// items by descending cost (longest-processing-time first; the tail is the lightest rows of the
-// lightest head). Everything here is integer work on the packed mask only.
+// per-head density). The pre-pass builds the work items and orders them:
+//   * an item is one query block or, for the tcgen05 kernel on large problems, a PAIR of query
+//     blocks of one (batch, head) that share every staged K/V tile. Adjacent blocks (2i, 2i+1)
+//     are paired when their popcounts are balanced (3D-local masks make neighbours share most key
+//     blocks). A block that is much heavier than its neighbour would run alone for most of the
+//     item (one softmax warpgroup idle), so both go to a pool instead; the pool is sorted by
+//     popcount and matched within windows of four rows by bit-row overlap (__popc(row_a & row_b)):
+//     heavy rows meet heavy rows (BASELINE.json's adversarial case: the fully dense rows pair up),
+//     and among equally heavy candidates the partner with the most shared key blocks wins.
+//   * (b,h) groups heaviest first (keeps the concurrently running CTAs on one or two heads, whose
+//     K/V then stay in L2) and, inside a group, items by descending cost (longest-processing-time
+//     first; the tail is the lightest items of the lightest head).
+// Everything here is integer work on the packed mask only; the resulting order cannot change any
+// output bit (each query block is reduced by one CTA over its key blocks in ascending order).
 #include "common.cuh"
 
 namespace sa {
 
 size_t fwd_workspace_bytes(int B, int H, int NQB) {
   const size_t BH = static_cast<size_t>(B) * H;
-  const size_t n = 16 + 3 * BH + 2 * BH * static_cast<size_t>(NQB);
-  return ((n * sizeof(int32_t) + 255) / 256) * 256;
+  const size_t words = 16 + 3 * BH + 4 * BH * static_cast<size_t>(NQB);   // two int2 arrays of BH*NQB records
+  return ((words * sizeof(int32_t) + 255) / 256) * 256;
 }
 
 FwdWorkspace carve_fwd_workspace(void* ws, int B, int H, int NQB) {
@@ -22,105 +32,208 @@ FwdWorkspace carve_fwd_workspace(void* ws, int B, int H, int NQB) {
   int32_t* p = static_cast<int32_t*>(ws);
   FwdWorkspace w;
   w.cursor = p;
+  w.n_items = p + 1;
   w.head_cost = p + 16;
-  w.head_order = w.head_cost + BH;
-  w.kmax2 = reinterpret_cast<float*>(w.head_order + BH);
-  w.local_order = w.head_order + 2 * BH;
-  w.unit_order = w.local_order + BH * static_cast<size_t>(NQB);
+  w.head_count = w.head_cost + BH;
+  w.kmax2 = reinterpret_cast<float*>(w.head_count + BH);
+  int32_t* rec = w.head_count + 2 * BH;
+  rec += (reinterpret_cast<uintptr_t>(rec) & 7u) ? 1 : 0;                 // int2 alignment (ws is 16 B aligned)
+  w.local_items = reinterpret_cast<int2*>(rec);
+  w.items = w.local_items + BH * static_cast<size_t>(NQB);
   return w;
 }
 
 namespace {
 
 constexpr int kSortThreads = 1024;
+constexpr uint32_t kIdxBits = 14, kIdxMask = (1u << kIdxBits) - 1u;       // rows / slots < 16384
 
-// grid = B*H blocks. Item i of group (b,h) covers query blocks [i*rpi, min((i+1)*rpi, NQB)); its
-// cost is the number of active (query block, key block) tiles in it. local_order[bh][pos] = item
-// with the pos-th largest cost (ties: lower item first).
+// shared-memory sort of s[0, n2), n2 a power of two, DESCENDING (zeros, the padding, end up last)
+__device__ void bitonic_sort_desc(uint32_t* s, int n2) {
+  for (int k = 2; k <= n2; k <<= 1) {
+    for (int j = k >> 1; j > 0; j >>= 1) {
+      for (int i = threadIdx.x; i < n2; i += blockDim.x) {
+        const int x = i ^ j;
+        if (x > i) {
+          const uint32_t a = s[i], b = s[x];
+          const bool desc = (i & k) == 0;
+          if (desc ? (a < b) : (a > b)) { s[i] = b; s[x] = a; }
+        }
+      }
+      __syncthreads();
+    }
+  }
+}
+
+__device__ __forceinline__ int pow2_at_least(int n) {
+  int p = 32;
+  while (p < n) p <<= 1;
+  return p;
+}
+
+// |row_a & row_b| over the W mask words; every lane of the warp returns the sum
+__device__ __forceinline__ int overlap(const uint32_t* __restrict__ ra, const uint32_t* __restrict__ rb,
+                                       int W, uint32_t tail_mask, int lane) {
+  int c = 0;
+  for (int w = lane; w < W; w += 32) {
+    uint32_t x = __ldg(ra + w) & __ldg(rb + w);
+    if (w == W - 1) x &= tail_mask;
+    c += __popc(x);
+  }
+  return __reduce_add_sync(0xFFFFFFFFu, c);
+}
+
+// grid = B*H blocks. Builds the items of group (b,h), sorted by cost (active tiles) descending:
+// local_items[bh][pos] = {cost, ua | ub << 16} (ub = 0xFFFF: single-row item); head_cost[bh] =
+// active tiles of the group; head_count[bh] = its number of items.
+// Dynamic shared memory: keys[n2] (uint32), then pop[NQB], ia[slots], ib[slots] (uint16).
 __global__ void __launch_bounds__(kSortThreads)
-schedule_sort_kernel(const uint32_t* __restrict__ mask_bits, int H, int NQB, int NKB, int W,
-                     int rpi, int items, int32_t* __restrict__ head_cost,
-                     int32_t* __restrict__ local_order, float* __restrict__ kmax2) {
-  extern __shared__ int32_t s_cost[];
-  __shared__ int s_total;
-  const int bh = blockIdx.x;
-  const int h = bh % H;
+schedule_items_kernel(const uint32_t* __restrict__ mask_bits, int H, int NQB, int NKB, int W,
+                      int pair_rows, int n2, int32_t* __restrict__ head_cost,
+                      int32_t* __restrict__ head_count, int2* __restrict__ local_items,
+                      float* __restrict__ kmax2) {
+  extern __shared__ uint32_t s_keys[];
+  const int slots = NQB + 2;
+  uint16_t* s_pop = reinterpret_cast<uint16_t*>(s_keys + n2);
+  uint16_t* s_a = s_pop + ((NQB + 1) & ~1);
+  uint16_t* s_b = s_a + slots;
+  __shared__ int s_total, s_pool, s_count;
+  const int bh = blockIdx.x, h = bh % H;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t* rows = mask_bits + static_cast<size_t>(h) * NQB * W;
+  const uint32_t tail_mask = (NKB & 31) ? ((1u << (NKB & 31)) - 1u) : 0xFFFFFFFFu;
   if (threadIdx.x == 0) {
     s_total = 0;
-    kmax2[bh] = 0.f;                 // key_norm_kernel (next on the stream) takes the max into it
+    s_pool = 0;
+    s_count = 0;
+    kmax2[bh] = 0.f;                 // the key-norm pass (next on the stream) takes the max into it
   }
+  for (int i = threadIdx.x; i < n2; i += blockDim.x) s_keys[i] = 0u;
+  for (int i = threadIdx.x; i < slots; i += blockDim.x) s_a[i] = s_b[i] = 0xFFFFu;
   __syncthreads();
-  const uint32_t tail_mask = (NKB & 31) ? ((1u << (NKB & 31)) - 1u) : 0xFFFFFFFFu;
+
+  // ---- popcount of every row (one warp per row, lanes over the words)
   int my_total = 0;
-  for (int i = threadIdx.x; i < items; i += blockDim.x) {
+  for (int r = warp; r < NQB; r += kSortThreads / 32) {
     int c = 0;
-    for (int r = i * rpi; r < min((i + 1) * rpi, NQB); ++r) {
-      const uint32_t* row = mask_bits + (static_cast<size_t>(h) * NQB + r) * W;
-      for (int w = 0; w < W; ++w) {
-        uint32_t x = __ldg(row + w);
-        if (w == W - 1) x &= tail_mask;
-        c += __popc(x);
+    for (int w = lane; w < W; w += 32) {
+      uint32_t x = __ldg(rows + static_cast<size_t>(r) * W + w);
+      if (w == W - 1) x &= tail_mask;
+      c += __popc(x);
+    }
+    c = __reduce_add_sync(0xFFFFFFFFu, c);
+    if (lane == 0) {
+      s_pop[r] = static_cast<uint16_t>(c);
+      my_total += c;
+    }
+  }
+  if (lane == 0) atomicAdd(&s_total, my_total);
+  __syncthreads();
+
+  const int n_adj = pair_rows ? NQB / 2 : 0;     // slots [0, n_adj): adjacent pairs; then pool pairs
+  if (pair_rows) {
+    // ---- adjacent pairs: kept when balanced (the lighter row has at least ~0.4 of the heavier
+    // one's tiles: below that, running the heavy row alone for most of the item costs more than
+    // the shared K/V tiles save), otherwise both rows go to the pool
+    for (int i = threadIdx.x; i < n_adj; i += blockDim.x) {
+      const int pa = s_pop[2 * i], pb = s_pop[2 * i + 1];
+      const int lo = min(pa, pb), hi = max(pa, pb);
+      if (5 * lo + 8 >= 2 * hi) {
+        s_a[i] = static_cast<uint16_t>(2 * i);
+        s_b[i] = static_cast<uint16_t>(2 * i + 1);
+      } else {
+        const int at = atomicAdd(&s_pool, 2);
+        s_keys[at] = (static_cast<uint32_t>(pa) << kIdxBits) | (kIdxMask - (2 * i));
+        s_keys[at + 1] = (static_cast<uint32_t>(pb) << kIdxBits) | (kIdxMask - (2 * i + 1));
       }
     }
-    s_cost[i] = c;
-    my_total += c;
-  }
-  atomicAdd(&s_total, my_total);
-  __syncthreads();
-  if (threadIdx.x == 0) head_cost[bh] = s_total;
-  for (int i = threadIdx.x; i < items; i += blockDim.x) {
-    const int ci = s_cost[i];
-    int pos = 0;
-    for (int j = 0; j < items; ++j) {
-      const int cj = s_cost[j];
-      pos += (cj > ci) || (cj == ci && j < i);
+    if (threadIdx.x == 0 && (NQB & 1)) {
+      const int at = atomicAdd(&s_pool, 1);
+      s_keys[at] = (static_cast<uint32_t>(s_pop[NQB - 1]) << kIdxBits) | (kIdxMask - (NQB - 1));
     }
-    local_order[static_cast<size_t>(bh) * items + pos] = i;
+    __syncthreads();
+    const int P = s_pool;
+    if (P > 0) {
+      // ---- pool: popcount descending (ties: lower row first; the keys are unique, so the order
+      // does not depend on the order of the atomics above)
+      bitonic_sort_desc(s_keys, pow2_at_least(P));
+      // windows of four rows: of the three ways to split {0,1,2,3} into two pairs take the one
+      // with the largest total overlap; a last window of 1-3 rows pairs in order
+      for (int g = warp; 4 * g < P; g += kSortThreads / 32) {
+        int r[4];
+        for (int i = 0; i < 4; ++i)
+          r[i] = 4 * g + i < P ? static_cast<int>(kIdxMask - (s_keys[4 * g + i] & kIdxMask)) : -1;
+        int p0 = 1, p1 = 2, p2 = 3;              // partner of row 0; the remaining two rows
+        if (r[3] >= 0) {
+          const uint32_t* m0 = rows + static_cast<size_t>(r[0]) * W;
+          const uint32_t* m1 = rows + static_cast<size_t>(r[1]) * W;
+          const uint32_t* m2 = rows + static_cast<size_t>(r[2]) * W;
+          const uint32_t* m3 = rows + static_cast<size_t>(r[3]) * W;
+          const int o01 = overlap(m0, m1, W, tail_mask, lane), o23 = overlap(m2, m3, W, tail_mask, lane);
+          const int o02 = overlap(m0, m2, W, tail_mask, lane), o13 = overlap(m1, m3, W, tail_mask, lane);
+          const int o03 = overlap(m0, m3, W, tail_mask, lane), o12 = overlap(m1, m2, W, tail_mask, lane);
+          int best = o01 + o23;
+          if (o02 + o13 > best) { best = o02 + o13; p0 = 2; p1 = 1; p2 = 3; }
+          if (o03 + o12 > best) { p0 = 3; p1 = 1; p2 = 2; }
+        }
+        if (lane == 0) {
+          const int s = n_adj + 2 * g;
+          s_a[s] = static_cast<uint16_t>(r[0]);
+          s_b[s] = r[p0] >= 0 ? static_cast<uint16_t>(r[p0]) : 0xFFFFu;
+          if (r[p1] >= 0) {
+            s_a[s + 1] = static_cast<uint16_t>(r[p1]);
+            s_b[s + 1] = r[p2] >= 0 ? static_cast<uint16_t>(r[p2]) : 0xFFFFu;
+          }
+        }
+      }
+      __syncthreads();
+      for (int i = threadIdx.x; i < n2; i += blockDim.x) s_keys[i] = 0u;
+      __syncthreads();
+    }
+  } else {
+    for (int i = threadIdx.x; i < NQB; i += blockDim.x) s_a[i] = static_cast<uint16_t>(i);
+    __syncthreads();
+  }
+
+  // ---- items by cost descending (ties: lower slot first); empty slots keep key 0 and sort last
+  const int used = pair_rows ? n_adj + (NQB - 2 * n_adj + 2 * n_adj + 1) / 2 + 1 : NQB;   // upper bound of slots in use
+  int mine = 0;
+  for (int s = threadIdx.x; s < min(used, slots); s += blockDim.x) {
+    const int a = s_a[s], b = s_b[s];
+    if (a == 0xFFFF) continue;
+    const int cost = s_pop[a] + (b != 0xFFFF ? s_pop[b] : 0);
+    s_keys[s] = (static_cast<uint32_t>(cost + 1) << kIdxBits) | (kIdxMask - s);
+    ++mine;
+  }
+  if (mine) atomicAdd(&s_count, mine);
+  __syncthreads();
+  bitonic_sort_desc(s_keys, n2);
+  const int count = s_count;
+  for (int pos = threadIdx.x; pos < count; pos += blockDim.x) {
+    const uint32_t key = s_keys[pos];
+    const int s = static_cast<int>(kIdxMask - (key & kIdxMask));
+    local_items[static_cast<size_t>(bh) * NQB + pos] =
+        make_int2(static_cast<int>(key >> kIdxBits) - 1, s_a[s] | (static_cast<int>(s_b[s]) << 16));
+  }
+  if (threadIdx.x == 0) {
+    head_cost[bh] = s_total;
+    head_count[bh] = count;
   }
 }
 
-// unit_order[p] = global item id (bh * items + local item) issued p-th; resets the cursor.
-// Every block first ranks the (b,h) groups by (cost descending, id ascending) into shared memory.
-__global__ void __launch_bounds__(256)
-schedule_flatten_kernel(const int32_t* __restrict__ head_cost, int32_t* __restrict__ head_order,
-                        const int32_t* __restrict__ local_order, int BH, int items,
-                        int32_t* __restrict__ unit_order, int32_t* __restrict__ cursor) {
-  extern __shared__ int32_t s_order[];
-  for (int g = threadIdx.x; g < BH; g += blockDim.x) {
-    const int cg = __ldg(head_cost + g);
-    int ahead = 0;
-    for (int j = 0; j < BH; ++j) {
-      const int cj = __ldg(head_cost + j);
-      ahead += (cj > cg) || (cj == cg && j < g);
-    }
-    s_order[ahead] = g;
-  }
-  __syncthreads();
-  const int p = blockIdx.x * blockDim.x + threadIdx.x;
-  if (p == 0) *cursor = 0;
-  if (p >= BH * items) return;
-  const int rank = p / items, pos = p % items;
-  const int bh = s_order[rank];
-  if (pos == 0) head_order[rank] = bh;
-  unit_order[p] = bh * items + local_order[static_cast<size_t>(bh) * items + pos];
-}
-
-// kmax2[bh] = max over the valid keys j of |k_j|^2 (D = 128). Half a warp per key row: 16 lanes x 16
-// bytes = one 256 B row per load, fully coalesced; 4 shuffles fold the 16 partial sums.
+// kmax2[bh] = max over the valid keys j of |k_j|^2 (D = 128), rows [r0, r1). Half a warp per key row:
+// 16 lanes x 16 bytes = one 256 B row per load, fully coalesced; 4 shuffles fold the 16 partial sums.
 // The forward kernel turns it into the Cauchy-Schwarz bound scale * |q_i| * max_j |k_j| >= every
 // score of query row i, which lets it fix the softmax reference point of a row for a whole item.
-constexpr int kNormThreads = 256;
+constexpr int kFlatThreads = 256;
 constexpr int kNormRowsPerBlock = 1024;
-__global__ void __launch_bounds__(kNormThreads)
-key_norm_kernel(const __nv_bfloat16* __restrict__ k, int N, int n_valid, float* __restrict__ kmax2) {
-  const int bh = blockIdx.y;
-  const int r0 = blockIdx.x * kNormRowsPerBlock;
-  const int r1 = min(r0 + kNormRowsPerBlock, n_valid);
+__device__ __forceinline__ void key_norm_slice(const __nv_bfloat16* __restrict__ k, int N, int r0, int r1,
+                                               int bh, float* __restrict__ kmax2) {
   const int half = threadIdx.x >> 4, sub = threadIdx.x & 15;       // 16 half-warps per block
   const uint4* base = reinterpret_cast<const uint4*>(k + static_cast<size_t>(bh) * N * 128);
   float best = 0.f;
 #pragma unroll 4
-  for (int rb = r0; rb < r1; rb += kNormThreads / 16) {       // uniform trip count (shuffles inside)
+  for (int rb = r0; rb < r1; rb += kFlatThreads / 16) {       // uniform trip count (shuffles inside)
     const int r = rb + half;
     const uint4 x = r < r1 ? __ldg(base + static_cast<size_t>(r) * 16 + sub) : make_uint4(0u, 0u, 0u, 0u);
     const uint32_t w[4] = {x.x, x.y, x.z, x.w};
@@ -138,6 +251,58 @@ key_norm_kernel(const __nv_bfloat16* __restrict__ k, int N, int n_valid, float* 
   best = fmaxf(best, __shfl_xor_sync(0xFFFFFFFFu, best, 16));
   if ((threadIdx.x & 31) == 0)
     atomicMax(reinterpret_cast<unsigned*>(kmax2 + bh), __float_as_uint(best));   // non-negative floats
+}
+
+// grid = (X, B*H). Block (x, bh): (1) if `flatten`, copies items [256 x, 256 x + 256) of group bh to
+// their place in the issue order -- the groups go heaviest first (ties: lower id), so the group's
+// first item sits at the sum of the item counts of the groups ahead of it, which every copying block
+// works out for itself in O(B*H / 256) steps; block (0,0) also zeroes the cursor and publishes the
+// total item count; (2) if `k` is given, takes key rows [1024 x, 1024 x + 1024) of the group into
+// kmax2[bh] (one launch instead of two: the forward call is launch-latency bound on short sequences).
+__global__ void __launch_bounds__(kFlatThreads)
+schedule_flatten_kernel(const int32_t* __restrict__ head_cost, const int32_t* __restrict__ head_count,
+                        const int2* __restrict__ local_items, int BH, int NQB, int flatten,
+                        int2* __restrict__ items, int32_t* __restrict__ cursor,
+                        int32_t* __restrict__ n_items, const __nv_bfloat16* __restrict__ k, int N,
+                        int n_valid, float* __restrict__ kmax2) {
+  const int bh = blockIdx.y;
+  if (flatten) {
+    const int count = __ldg(head_count + bh);
+    const bool first = blockIdx.x == 0 && bh == 0;
+    if (static_cast<int>(blockIdx.x) * kFlatThreads < count || first) {
+      __shared__ int s_start, s_all;
+      if (threadIdx.x == 0) s_start = s_all = 0;
+      __syncthreads();
+      const int cg = __ldg(head_cost + bh);
+      int start = 0, all = 0;
+      for (int j = threadIdx.x; j < BH; j += kFlatThreads) {
+        const int cj = __ldg(head_cost + j), nj = __ldg(head_count + j);
+        all += nj;
+        if (cj > cg || (cj == cg && j < bh)) start += nj;
+      }
+      start = __reduce_add_sync(0xFFFFFFFFu, start);
+      all = __reduce_add_sync(0xFFFFFFFFu, all);
+      if ((threadIdx.x & 31) == 0) {
+        atomicAdd(&s_start, start);
+        atomicAdd(&s_all, all);
+      }
+      __syncthreads();
+      const int pos = blockIdx.x * kFlatThreads + threadIdx.x;
+      if (pos < count) {
+        const int2 rec = __ldg(local_items + static_cast<size_t>(bh) * NQB + pos);
+        items[s_start + pos] = make_int2(bh, rec.y);
+      }
+      if (first && threadIdx.x == 0) {
+        *cursor = 0;
+        *n_items = s_all;
+      }
+    }
+  }
+  if (k != nullptr) {
+    const int r0 = blockIdx.x * kNormRowsPerBlock;
+    const int r1 = min(r0 + kNormRowsPerBlock, n_valid);
+    if (r0 < r1) key_norm_slice(k, N, r0, r1, bh, kmax2);
+  }
 }
 
 __global__ void __launch_bounds__(128)
@@ -158,23 +323,33 @@ enumerate_kernel(const uint32_t* __restrict__ mask_bits, int rows, int NKB, int 
 cudaError_t launch_schedule(const FwdParams& p, const FwdWorkspace& w, int rpi, cudaStream_t st,
                             int* n_launch, bool reuse) {
   const int BH = p.B * p.H;
-  const int items = (p.NQB + rpi - 1) / rpi;
+  const bool norms = p.D == 128 && p.kmax2 != nullptr;   // the tcgen05 kernel's score bound needs max |k|^2
+  cudaError_t e;
   if (reuse) {
     // the work list in the workspace is still valid (same mask): only reset what a call consumes
-    cudaError_t e = cudaMemsetAsync(w.cursor, 0, sizeof(int32_t), st);
-    if (e == cudaSuccess) e = cudaMemsetAsync(w.kmax2, 0, static_cast<size_t>(BH) * sizeof(float), st);
+    e = cudaMemsetAsync(w.cursor, 0, sizeof(int32_t), st);
+    if (e == cudaSuccess && norms) e = cudaMemsetAsync(w.kmax2, 0, static_cast<size_t>(BH) * sizeof(float), st);
     if (e != cudaSuccess) return e;
   } else {
-  schedule_sort_kernel<<<BH, kSortThreads, items * sizeof(int32_t), st>>>(
-      p.mask_bits, p.H, p.NQB, p.NKB, p.W, rpi, items, w.head_cost, w.local_order, w.kmax2);
-  const int total = BH * items;
-  schedule_flatten_kernel<<<(total + 255) / 256, 256, BH * sizeof(int32_t), st>>>(
-      w.head_cost, w.head_order, w.local_order, BH, items, w.unit_order, w.cursor);
-  *n_launch += 2;
+    int n2 = 32;
+    while (n2 < p.NQB + 2) n2 <<= 1;
+    const size_t smem = static_cast<size_t>(n2) * 4 + (static_cast<size_t>((p.NQB + 1) & ~1) + 2 * (p.NQB + 2)) * 2;
+    if (smem > 48 * 1024) {
+      e = ensure_dynamic_smem(kSmemScheduleItems, reinterpret_cast<const void*>(schedule_items_kernel),
+                              200 * 1024);
+      if (e != cudaSuccess) return e;
+    }
+    schedule_items_kernel<<<BH, kSortThreads, smem, st>>>(p.mask_bits, p.H, p.NQB, p.NKB, p.W, rpi == 2 ? 1 : 0,
+                                                         n2, w.head_cost, w.head_count, w.local_items, w.kmax2);
+    *n_launch += 1;
   }
-  if (p.D == 128 && p.kmax2 != nullptr) {   // the tcgen05 kernel's score bound needs max |k|^2
-    const dim3 grid((p.n_valid + kNormRowsPerBlock - 1) / kNormRowsPerBlock, BH);
-    key_norm_kernel<<<grid, kNormThreads, 0, st>>>(p.k, p.N, p.n_valid, w.kmax2);
+  if (!reuse || norms) {
+    const int xf = reuse ? 0 : (p.NQB + kFlatThreads - 1) / kFlatThreads;
+    const int xn = norms ? (p.n_valid + kNormRowsPerBlock - 1) / kNormRowsPerBlock : 0;
+    const dim3 grid(xf > xn ? xf : xn, BH);
+    schedule_flatten_kernel<<<grid, kFlatThreads, 0, st>>>(w.head_cost, w.head_count, w.local_items, BH, p.NQB,
+                                                          reuse ? 0 : 1, w.items, w.cursor, w.n_items,
+                                                          norms ? p.k : nullptr, p.N, p.n_valid, w.kmax2);
     *n_launch += 1;
   }
   return cudaGetLastError();

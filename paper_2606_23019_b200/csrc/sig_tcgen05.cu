@@ -253,19 +253,12 @@ sig_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
 cudaError_t launch_block_significance(const __nv_bfloat16* q, const __nv_bfloat16* k, const float* lse,
                                       float* sig, int B, int H, int N, int n_valid, float scale,
                                       cudaStream_t st, const char** err_text) {
-  static int n_sm = 0;
-  static bool attr_set = false;
-  if (!attr_set) {
-    int dev = 0;
-    cudaError_t e = cudaGetDevice(&dev);
-    if (e != cudaSuccess) return e;
-    e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(sig_tcgen05_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             static_cast<int>(kSmemBytes));
-    if (e != cudaSuccess) { *err_text = "cudaFuncSetAttribute(sig_tcgen05_kernel)"; return e; }
-    attr_set = true;
-  }
+  int n_sm = 0;
+  cudaError_t e = device_sm_count(&n_sm);
+  if (e != cudaSuccess) return e;
+  e = ensure_dynamic_smem(kSmemSigTcgen05, reinterpret_cast<const void*>(sig_tcgen05_kernel),
+                          static_cast<int>(kSmemBytes));
+  if (e != cudaSuccess) { *err_text = "cudaFuncSetAttribute(sig_tcgen05_kernel)"; return e; }
   CUtensorMap tq, tk;
   const uint64_t rows = static_cast<uint64_t>(B) * H * N;
   if (!make_tile_map_128x64(&tq, q, rows) || !make_tile_map_128x64(&tk, k, rows)) {
