@@ -220,9 +220,28 @@ SA_API sa_status sa_enumerate_active_blocks(const uint32_t* mask_bits, int H, in
  * second CUDA implementation kept for cross-checking; not a fallback: it is never chosen implicitly
  * for a shape the fast kernel supports). 2 / 3: the tcgen05 kernel with its large-problem path (pair
  * items, key-norm pre-pass and score bound) / its small-problem path (single-block items, exact running
- * max) forced, so that tests can drive either on any size. Process-wide. */
+ * max) forced, so that tests can drive either on any size. A DEBUG hook for tests and benchmarks, not
+ * part of the product surface: process-wide (an atomic read once per call), so it must not be changed
+ * while another thread is inside a forward call. The same holds for sa_profile_enable / _collect. */
 SA_API sa_status sa_set_fwd_variant(int variant);
 SA_API int sa_get_fwd_variant(void);
+
+/* Debug hook: sa_block_sparse_attn_fwd_ex on a build of the (128,128,128) tcgen05 kernel that also
+ * records its walk, so that the union walk of a work item (Alg. 2 re-expressed over the OR of two
+ * bit-rows), the numbering of (tile, key block) units and the 64-word window reload can be checked
+ * index by index against a CPU enumeration. walk_log: device int32, sa_debug_fwd_walk_log_bytes(...)
+ * bytes, zero-filled by the caller. With R = B*H*N/Bq rows (row = (b*H + h)*NQB + u) and NKB = N/Bk:
+ *   wg_cnt [R]           units the softmax warpgroup of the row's tile consumed
+ *   wg_info[R]           (partner + 1) << 1 | tile      (partner = the item's other query block, -1: none)
+ *   wg_seq [R][NKB]      unit << 16 | key block, in consumption order (unit = number in the item's walk)
+ *   is_cnt [R]           units the MMA issuer issued for the item whose tile 0 is this row
+ *   is_seq [R][2*NKB]    tile << 15 | key block, in issue order
+ * Results (out, lse) are those of the product kernel. Requires (D,Bq,Bk) = (128,128,128). */
+SA_API size_t sa_debug_fwd_walk_log_bytes(int B, int H, int N, int Bq, int Bk);
+SA_API sa_status sa_debug_fwd_walk(const void* q, const void* k, const void* v, const uint32_t* mask_bits,
+                                   void* out, float* lse, int B, int H, int N, int n_valid, int D, int Bq,
+                                   int Bk, float scale, void* workspace, size_t workspace_bytes,
+                                   int32_t* walk_log, size_t walk_log_bytes, void* stream);
 
 /* Number of kernels the last sa_pack_mask / forward / sa_hot_path_host call on this thread
  * enqueued (for bench accounting; memsets and copies are not counted). */

@@ -6,6 +6,7 @@ loaded, or a call returns a non-OK status, SAError is raised.
 """
 from __future__ import annotations
 
+import contextlib
 import ctypes as C
 import os
 
@@ -14,6 +15,7 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libscalingattn.so")
 _lib = None
+_null_ctx = contextlib.nullcontext
 
 SA_OK = 0
 
@@ -68,6 +70,11 @@ def load_library() -> C.CDLL:
                                                 fp, vp, sz, vp]
     lib.sa_block_sparse_attn_fwd_reuse.restype = ip
     lib.sa_block_sparse_attn_fwd_reuse.argtypes = lib.sa_block_sparse_attn_fwd_ex.argtypes
+    lib.sa_debug_fwd_walk_log_bytes.restype = sz
+    lib.sa_debug_fwd_walk_log_bytes.argtypes = [ip] * 5
+    lib.sa_debug_fwd_walk.restype = ip
+    lib.sa_debug_fwd_walk.argtypes = [vp, vp, vp, vp, vp, vp, ip, ip, ip, ip, ip, ip, ip, fp, vp, sz,
+                                      vp, sz, vp]
     lib.sa_block_sparse_attn_fwd_host.restype = ip
     lib.sa_block_sparse_attn_fwd_host.argtypes = [vp, vp, vp, vp, vp, vp, ip, ip, ip, ip, ip, ip,
                                                   ip, fp, vp, sz, vp]
@@ -278,6 +285,32 @@ def sa_block_sparse_attn_fwd_ex(q, k, v, mask_bits, Bq: int, Bk: int, scale: flo
                                            _ptr(lse), B, H, N, n_valid, D, Bq, Bk, float(scale),
                                            _ptr(workspace), workspace.numel(), _stream(stream)))
     return out, lse
+
+
+def sa_debug_fwd_walk(q, k, v, mask_bits, Bq: int, Bk: int, scale: float, n_valid=None, stream=None):
+    """Debug hook (include/scalingattn.h): the forward call on the walk-recording build of the tcgen05
+    kernel. Returns out, lse and the log regions as int32 tensors
+    (wg_cnt [R], wg_info [R], wg_seq [R][NKB], is_cnt [R], is_seq [R][2*NKB]), R = B*H*N/Bq."""
+    lib = load_library()
+    B, H, N, D = _fwd_shapes(q, k, v, mask_bits, Bq, Bk)
+    n_valid = N if n_valid is None else int(n_valid)
+    out = torch.empty_like(q)
+    lse = torch.empty((B, H, N), dtype=torch.float32, device=q.device)
+    with torch.cuda.stream(stream) if stream is not None else _null_ctx():
+        workspace = torch.empty(max(lib.sa_fwd_workspace_bytes(B, H, N, Bq), 256), dtype=torch.uint8,
+                                device=q.device)
+        log = torch.zeros(lib.sa_debug_fwd_walk_log_bytes(B, H, N, Bq, Bk) // 4, dtype=torch.int32,
+                          device=q.device)
+    _check(lib.sa_debug_fwd_walk(_ptr(q), _ptr(k), _ptr(v), _ptr(mask_bits), _ptr(out), _ptr(lse), B, H, N,
+                                 n_valid, D, Bq, Bk, float(scale), _ptr(workspace), workspace.numel(),
+                                 _ptr(log), log.numel() * 4, _stream(stream)))
+    R, NKB = B * H * (N // Bq), N // Bk
+    o = 0
+    regions = []
+    for n, shape in ((R, (R,)), (R, (R,)), (R * NKB, (R, NKB)), (R, (R,)), (2 * R * NKB, (R, 2 * NKB))):
+        regions.append(log[o:o + n].view(shape))
+        o += n
+    return (out, lse) + tuple(regions)
 
 
 def sa_block_sparse_attn_fwd_host(q, k, v, mask_bits, out, lse, Bq: int, Bk: int, scale: float,

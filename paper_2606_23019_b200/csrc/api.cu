@@ -267,7 +267,8 @@ sa_status sa_fidelity_from_lse(const float* lse_dense, const float* lse_sparse, 
 static sa_status fwd_ex_impl(const void* q, const void* k, const void* v, const uint32_t* mask_bits,
                              void* out, float* lse, int B, int H, int N, int n_valid, int D, int Bq,
                              int Bk, float scale, void* workspace, size_t workspace_bytes, void* stream,
-                             bool mask_word_aligned, bool reuse_schedule = false) {
+                             bool mask_word_aligned, bool reuse_schedule = false,
+                             int32_t* walk_log = nullptr) {
   g_last_launches = 0;
   if (!q || !k || !v || !mask_bits || !out || !lse)
     return fail(SA_ERR_INVALID_ARG, "sa_block_sparse_attn_fwd: null pointer");
@@ -301,7 +302,8 @@ static sa_status fwd_ex_impl(const void* q, const void* k, const void* v, const 
   p.items = w.items;
   p.n_items_dev = w.n_items;
   p.counter = w.cursor;
-  const int variant = g_variant.load(std::memory_order_relaxed);
+  p.walk_log = walk_log;
+  const int variant = walk_log ? 2 : g_variant.load(std::memory_order_relaxed);   // the walk log is the pair path's
   const bool fast = (variant != 1 && D == 128);
   // the per-row score bound saves ~6% of the attention kernel but costs one more (~8 us) launch:
   // not worth it on problems of a few thousand tiles, which then keep the exact running max
@@ -350,6 +352,25 @@ sa_status sa_block_sparse_attn_fwd_ex(const void* q, const void* k, const void* 
                                       void* stream) {
   return fwd_ex_impl(q, k, v, mask_bits, out, lse, B, H, N, n_valid, D, Bq, Bk, scale, workspace,
                      workspace_bytes, stream, false);
+}
+
+size_t sa_debug_fwd_walk_log_bytes(int B, int H, int N, int Bq, int Bk) {
+  if (B <= 0 || H <= 0 || N <= 0 || Bq <= 0 || Bk <= 0 || N % Bq || N % Bk) return 0;
+  const size_t rows = static_cast<size_t>(B) * H * (N / Bq), nkb = static_cast<size_t>(N / Bk);
+  return (3 * rows + 3 * rows * nkb) * sizeof(int32_t);
+}
+
+sa_status sa_debug_fwd_walk(const void* q, const void* k, const void* v, const uint32_t* mask_bits,
+                            void* out, float* lse, int B, int H, int N, int n_valid, int D, int Bq,
+                            int Bk, float scale, void* workspace, size_t workspace_bytes,
+                            int32_t* walk_log, size_t walk_log_bytes, void* stream) {
+  if (D != 128 || Bq != 128 || Bk != 128)
+    return fail(SA_ERR_UNSUPPORTED, "sa_debug_fwd_walk: only (D,Bq,Bk) = (128,128,128)");
+  const size_t need = sa_debug_fwd_walk_log_bytes(B, H, N, Bq, Bk);
+  if (!walk_log || need == 0 || walk_log_bytes < need)
+    return fail(SA_ERR_WORKSPACE, "sa_debug_fwd_walk: walk_log %zu B < %zu B", walk_log_bytes, need);
+  return fwd_ex_impl(q, k, v, mask_bits, out, lse, B, H, N, n_valid, D, Bq, Bk, scale, workspace,
+                     workspace_bytes, stream, false, false, walk_log);
 }
 
 sa_status sa_block_sparse_attn_fwd_reuse(const void* q, const void* k, const void* v,

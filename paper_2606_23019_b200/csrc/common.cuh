@@ -66,6 +66,7 @@ struct FwdParams {
   const float* kmax2;         // [B*H] max |k|^2 over the valid keys (tcgen05 kernel only)
   int n_items;                // host-side count: exact for single-row items, an upper bound for pairs
   int rows_per_item;          // query blocks per work item: 2 (a pair shares its K/V tiles) or 1
+  int32_t* walk_log;          // sa_debug_fwd_walk only (else null): see WalkLog in fwd_tcgen05.cu
 };
 
 // Workspace layout for the forward pass (int32 words):
@@ -90,7 +91,7 @@ FwdWorkspace carve_fwd_workspace(void* ws, int B, int H, int NQB);
 
 // per-device state (device.cu): SM count of the current device; dynamic shared-memory opt-in of a
 // kernel, set once per (device, kernel)
-enum SmemKernel { kSmemFwdTcgen05 = 0, kSmemSigTcgen05, kSmemScheduleItems, kSmemFwdMmaSync64,
+enum SmemKernel { kSmemFwdTcgen05 = 0, kSmemFwdTcgen05Log, kSmemSigTcgen05, kSmemScheduleItems, kSmemFwdMmaSync64,
                   kSmemFwdMmaSync128, kNumSmemKernels };
 cudaError_t device_sm_count(int* n_sm);
 cudaError_t ensure_dynamic_smem(SmemKernel id, const void* func, int bytes);

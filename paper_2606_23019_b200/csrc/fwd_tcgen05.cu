@@ -46,7 +46,10 @@ constexpr int kD = 128;
 constexpr int kThreads = 384;
 constexpr uint32_t kTileBytes = kBlk * kD * 2;      // 32 KB
 constexpr uint32_t kHalfBytes = kTileBytes / 2;     // one [128][64] swizzle-128B box
-constexpr int kSlots = 5;                 // K/V ring
+#ifndef SA_SLOTS
+#define SA_SLOTS 5
+#endif
+constexpr int kSlots = SA_SLOTS;          // K/V ring
 constexpr int kSched = 2;                 // scheduler ring
 constexpr int kClaimAheadUnits = 512;     // items up to this many (tile, key block) units claim their successor early
 constexpr uint32_t kTmemCols = 512;
@@ -120,6 +123,24 @@ __device__ __forceinline__ Item decode_item(const FwdParams& p, int2 rec) {
   it.row0 = it.bh * p.N;
   return it;
 }
+
+// Debug log of the walk (sa_debug_fwd_walk; p.walk_log is null in every other call and the product
+// kernel is compiled without these stores). int32 regions, rows indexed by b*H*NQB + h*NQB + u:
+//   wg_cnt[rows], wg_info[rows] = (partner + 1) << 1 | tile, wg_seq[rows][NKB] = unit << 16 | key block
+//   (what the softmax warpgroup of the row's tile consumed, unit = number in the item's walk order),
+//   is_cnt[rows], is_seq[rows][2*NKB] = tile << 15 | key block (what the MMA issuer issued for the
+//   item whose tile 0 is this row, in issue order).
+struct WalkLog {
+  int32_t* base;
+  size_t rows, nkb;
+  __device__ explicit WalkLog(const FwdParams& p)
+      : base(p.walk_log), rows(static_cast<size_t>(p.B) * p.H * p.NQB), nkb(p.NKB) {}
+  __device__ int32_t* wg_cnt() const { return base; }
+  __device__ int32_t* wg_info() const { return base + rows; }
+  __device__ int32_t* wg_seq(size_t row) const { return base + 2 * rows + row * nkb; }
+  __device__ int32_t* is_cnt() const { return base + 2 * rows + rows * nkb; }
+  __device__ int32_t* is_seq(size_t row) const { return base + 3 * rows + rows * nkb + row * 2 * nkb; }
+};
 
 // word w of the bit-row of query block u (0 beyond the grid), stray high bits cleared
 __device__ __forceinline__ uint32_t row_word(const FwdParams& p, int h, int u, int w, bool exists) {
@@ -278,6 +299,7 @@ struct Pend {
 // tiles has still ping-pongs between the two S buffers. Issue order: PV(w-2), S(w): the softmax of
 // unit w-1 overlaps both. P(w-2) aliases S buffer (w & 1), so S(w) must follow PV(w-2) in the
 // (in-order) tensor pipe, which this order guarantees.
+template <bool kLog>
 __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uint32_t tmem,
                            int lane) {
   Ring ring;
@@ -343,6 +365,7 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
       rem[1] += n1;
     }
     bool first[2] = {true, true};
+    [[maybe_unused]] int n_logged = 0;
 
     // The next Q tiles are loaded only after every softmax warp has read the current ones (row
     // norms), and a softmax warp may be waiting for o_full of a unit still parked in the FIFO: if Q
@@ -358,6 +381,7 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     // descriptors) is done right after the first half of the current block's last S has been
     // issued, i.e. while the tensor pipe still has those MMAs queued, not between two units.
     struct Blk {
+      int j;                             // key block
       bool valid, has0, has1;
       uint32_t k_full, kphase, k_empty, v_full, vphase, v_empty;
       uint64_t kdesc, vdesc;
@@ -377,6 +401,7 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
       const int bit = __ffs(bx) - 1;
       bx &= bx - 1u;
       b.valid = true;
+      b.j = bw * 32 + bit;
       b.has0 = ((bx0 >> bit) & 1u) != 0;
       b.has1 = ((bx1 >> bit) & 1u) != 0;
       const int kslot = ring.slot;
@@ -421,6 +446,10 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
         const uint32_t tmem_s = tmem + buf * 128;
         const uint64_t qdesc = make_desc(kDescKMajor, smem_base + kOffQ + t * kTileBytes);
         const uint32_t s_full = bar(&ctl->s_full[t][sel]);
+        if constexpr (kLog) {          // debug build of the kernel (sa_debug_fwd_walk): the issue order
+          if (lane == 0) WalkLog(p).is_seq(it.bh * p.NQB + it.ua)[n_logged] = (t << 15) | cb.j;
+          ++n_logged;
+        }
         ++nt[t];
         if (first[t]) ++n_started[t];
         first[t] = false;
@@ -450,6 +479,9 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
       }
       tc_commit_e(cb.k_empty);
       cb = nb;
+    }
+    if constexpr (kLog) {
+      if (lane == 0) WalkLog(p).is_cnt()[it.bh * p.NQB + it.ua] = n_logged;
     }
     tc_commit_e(smem_u32(&ctl->q_empty));   // every S of this item has been issued
     // No S can follow until the next item's Q tiles have arrived, and their load starts only now:
@@ -518,6 +550,7 @@ __device__ __forceinline__ float exp_tile(const uint32_t (&sr)[4][32], float c, 
 // ------------------------------------------------------------------ warps 4-11: softmax + epilogue
 // One thread per query row: thread (quarter, lane) of warpgroup t owns TMEM lane 32*quarter+lane
 // of S_t / O_t, so row max and row sum need no shuffles.
+template <bool kLog>
 __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uint32_t tmem, int t,
                            int quarter, int lane) {
   const int row = quarter * 32 + lane;
@@ -601,6 +634,8 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     bool started = false;
     bool fixed = false;                  // warp-uniform: m_run is the bound, fixed for the item
     uint32_t prev_unit = 0xFFFFFFFEu;    // this tile's previous unit in the item
+    [[maybe_unused]] const uint32_t wg_item0 = wg;
+    [[maybe_unused]] int n_logged = 0;
     // Walk this tile's own bit-row. A unit's number in the union walk order (which the MMA issuer
     // follows) is the popcount of both rows below its bit. The next unit's bookkeeping is computed
     // in the same straight-line block as the exponentials, so it does not sit in the cycle
@@ -618,6 +653,12 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
                     (t == 1 ? (x0 >> bit) & 1u : 0u);
       for (;;) {
         const int j = w * 32 + bit;
+        if constexpr (kLog) {
+          if (quarter == 0 && lane == 0)
+            WalkLog(p).wg_seq(static_cast<size_t>(it.bh) * p.NQB + (t == 0 ? it.ua : it.ub))[n_logged] =
+                static_cast<int32_t>(((my - wg_item0) << 16) | static_cast<uint32_t>(j));
+          ++n_logged;
+        }
         const uint32_t buf = my & 1u, sel = nmine & 1u, par = (nmine >> 1) & 1u;
         const uint32_t tm_s = tmem + lane_base + buf * 128;
         SA_TR(0);
@@ -704,6 +745,14 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     }
 
     // ---- epilogue: O / l -> bf16, lse = ln2 * (m + log2 l); empty row -> 0 / -inf
+    if constexpr (kLog) {
+      if (exists && quarter == 0 && lane == 0) {
+        const size_t lrow = static_cast<size_t>(it.bh) * p.NQB + (t == 0 ? it.ua : it.ub);
+        const int partner = t == 0 ? (it.has1 ? it.ub : -1) : it.ua;
+        WalkLog(p).wg_cnt()[lrow] = n_logged;
+        WalkLog(p).wg_info()[lrow] = ((partner + 1) << 1) | t;
+      }
+    }
     const bool wrote = exists;
     const size_t grow = static_cast<size_t>(it.row0) + static_cast<size_t>(t == 0 ? it.ua : it.ub) * kBlk + row;
     uint4* orow = reinterpret_cast<uint4*>(p.out + grow * kD);
@@ -765,6 +814,7 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
 }
 
 // ------------------------------------------------------------------ kernel
+template <bool kLog>
 __global__ void __launch_bounds__(kThreads, 1)
 fwd_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
                    const __grid_constant__ CUtensorMap tm_v, const FwdParams p) {
@@ -815,11 +865,11 @@ fwd_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
     if (warp == 0) {
       producer(p, ctl, smem_base, &tm_q, &tm_k, &tm_v, lane);
     } else if (warp == 1) {
-      mma_issuer(p, ctl, smem_base, tmem, lane);
+      mma_issuer<kLog>(p, ctl, smem_base, tmem, lane);
     }
   } else {
     setmaxnreg_inc<208>();
-    softmax_wg(p, ctl, smem_base, tmem, warp >= 8 ? 1 : 0, warp & 3, lane);
+    softmax_wg<kLog>(p, ctl, smem_base, tmem, warp >= 8 ? 1 : 0, warp & 3, lane);
   }
   tc_fence_before();
   __syncthreads();
@@ -869,8 +919,11 @@ cudaError_t launch_fwd_tcgen05(const FwdParams& p, void*, cudaStream_t st, int* 
   int n_sm = 0;
   cudaError_t e = device_sm_count(&n_sm);
   if (e != cudaSuccess) return e;
-  e = ensure_dynamic_smem(kSmemFwdTcgen05, reinterpret_cast<const void*>(fwd_tcgen05_kernel),
-                          static_cast<int>(kSmemBytes));
+  const bool log = p.walk_log != nullptr;
+  e = log ? ensure_dynamic_smem(kSmemFwdTcgen05Log, reinterpret_cast<const void*>(fwd_tcgen05_kernel<true>),
+                                static_cast<int>(kSmemBytes))
+          : ensure_dynamic_smem(kSmemFwdTcgen05, reinterpret_cast<const void*>(fwd_tcgen05_kernel<false>),
+                                static_cast<int>(kSmemBytes));
   if (e != cudaSuccess) { *err_text = "cudaFuncSetAttribute(fwd_tcgen05_kernel)"; return e; }
   CUtensorMap tq, tk, tv;
   const uint64_t rows = static_cast<uint64_t>(p.B) * p.H * p.N;
@@ -879,7 +932,8 @@ cudaError_t launch_fwd_tcgen05(const FwdParams& p, void*, cudaStream_t st, int* 
     return cudaErrorInvalidValue;
   }
   const int grid = p.n_items < n_sm ? p.n_items : n_sm;   // n_items: upper bound (pairs are mask-dependent)
-  fwd_tcgen05_kernel<<<grid, kThreads, kSmemBytes, st>>>(tq, tk, tv, p);
+  if (log) fwd_tcgen05_kernel<true><<<grid, kThreads, kSmemBytes, st>>>(tq, tk, tv, p);
+  else fwd_tcgen05_kernel<false><<<grid, kThreads, kSmemBytes, st>>>(tq, tk, tv, p);
   *n_launch += 1;
   return cudaGetLastError();
 }

@@ -85,6 +85,77 @@ def test_device_bit_walk_matches_shift_and_test(sa, nkb):
             assert (idx[h, u, len(want):] == -1).all()
 
 
+@pytest.mark.parametrize("nkb", [20, 45, 591, 2048, 2100])      # W = 1, 2, 19, 64, 66 mask words per row
+def test_tcgen05_union_walk_matches_cpu_enumeration(sa, nkb):
+    # The tcgen05 kernel does not run Alg. 2 row by row: a work item walks the
+    # OR of two bit-rows, numbers its (tile, key block) units in walk order (ascending key block,
+    # tile 0 before tile 1), reloads the bit-rows in windows of 64 words, and the MMA issuer and the
+    # two softmax warpgroups each derive that numbering on their own. sa_debug_fwd_walk records
+    # what each of them did; the expected lists come from a shift-and-test walk of the same rows.
+    rng = np.random.Generator(np.random.PCG64(1000 + nkb))
+    H, nqb = 2, nkb
+    dense = rng.random((H, nqb, nkb)) < (0.25 if nkb <= 45 else 0.02)
+    dense[:, np.arange(nqb), np.arange(nqb)] = True
+    dense[0, 0] = False                         # empty row
+    dense[0, 1] = True                          # full row (next to an empty one: goes to the pool)
+    dense[1, 2] = False
+    dense[1, 2, nkb - 1] = True                 # single bit at the last position
+    dense[1, 3] = False
+    dense[1, 3, ::32] = True                    # one bit per word
+    bits = oracle.pack_bool(dense)
+    if nkb % 32:                                # stray bits past NKB are ignored
+        bits[1, :, -1] |= np.uint32((0xFFFFFFFF << (nkb % 32)) & 0xFFFFFFFF)
+    N = nkb * 128
+    g = torch.Generator(device="cuda").manual_seed(nkb)
+    q, k, v = [torch.randn((1, H, N, 128), generator=g, device="cuda", dtype=torch.float32).to(torch.bfloat16)
+               for _ in range(3)]
+    scale = float(np.float32(1 / math.sqrt(128)))
+    out, lse, wg_cnt, wg_info, wg_seq, is_cnt, is_seq = sa.sa_debug_fwd_walk(q, k, v, dev_bits(bits), 128, 128,
+                                                                            scale)
+    torch.cuda.synchronize()
+    # same bits as the product kernel on its pair path (variant 2 forces it at this size)
+    sa.sa_set_fwd_variant(2)
+    try:
+        out0, lse0 = sa.sa_block_sparse_attn_fwd_ex(q, k, v, dev_bits(bits), 128, 128, scale)
+    finally:
+        sa.sa_set_fwd_variant(0)
+    assert torch.equal(out, out0) and torch.equal(lse, lse0)
+    wg_cnt, wg_info, is_cnt = wg_cnt.cpu().numpy(), wg_info.cpu().numpy(), is_cnt.cpu().numpy()
+    wg_seq, is_seq = wg_seq.cpu().numpy(), is_seq.cpu().numpy()
+    seen = np.zeros((H, nqb), dtype=bool)
+    n_pairs = 0
+    for h in range(H):
+        for u in range(nqb):
+            r = h * nqb + u
+            t, partner = int(wg_info[r]) & 1, (int(wg_info[r]) >> 1) - 1
+            assert not seen[h, u]
+            seen[h, u] = True
+            a, b = (u, partner) if t == 0 else (partner, u)
+            assert a >= 0 and (b < 0 or (b != a and 0 <= b < nqb))
+            if b >= 0:                          # the partner names this row as its partner, other tile
+                rp = h * nqb + partner
+                assert (int(wg_info[rp]) >> 1) - 1 == u and (int(wg_info[rp]) & 1) == 1 - t
+                n_pairs += 1
+            # CPU enumeration of the item's walk from the boolean mask: key blocks ascending, tile 0
+            # before tile 1 on a key block both rows have; units numbered in that order
+            ja = np.nonzero(dense[h, a])[0]
+            jb = np.nonzero(dense[h, b])[0] if b >= 0 else np.zeros(0, dtype=np.int64)
+            js = np.concatenate([ja, jb])
+            ts = np.concatenate([np.zeros(len(ja), dtype=np.int64), np.ones(len(jb), dtype=np.int64)])
+            order = np.lexsort((ts, js))
+            js, ts = js[order], ts[order]
+            want_issue = (ts << 15) | js
+            mine = ts == t
+            want_mine = (np.arange(len(js))[mine] << 16) | js[mine]
+            assert wg_cnt[r] == len(want_mine), (h, u, wg_cnt[r], len(want_mine))
+            assert (wg_seq[r, :len(want_mine)] == np.asarray(want_mine, dtype=np.int64)).all(), (h, u)
+            if t == 0:
+                assert is_cnt[r] == len(want_issue), (h, u)
+                assert (is_seq[r, :len(want_issue)] == np.asarray(want_issue, dtype=np.int64)).all(), (h, u)
+    assert seen.all()                           # every query block belongs to exactly one item
+    assert n_pairs >= H * (nqb - 2)             # and all but an odd row per head are paired
+
+
 # ------------------------------------------------------------------ sa_pack_mask, bit-exact
 def _pack_both(sa, scores, density, force_diag):
     got = sa.sa_pack_mask(torch.from_numpy(scores).cuda(), torch.from_numpy(density).cuda(),
@@ -253,15 +324,22 @@ def test_score_bound_fallbacks(sa, case):
     bits = oracle.pack_bool(m)
     scale = float(np.float32(1 / math.sqrt(D)))
     ref_o, ref_l = oracle.attn(inputs.as_u16(q), inputs.as_u16(k), inputs.as_u16(v), bits, blk, blk, scale)
-    out, lse = run_fwd(sa, q, k, v, bits, blk, scale, variant=2)     # pair items (the big-problem path)
-    # lse is as large as the scores here: 1e-3 absolute is asked of O(10) values (BASELINE.json);
-    # allow the fp32 spacing of the value on top (|lse| up to ~1500 -> 1.2e-4 per ulp)
-    err = np.abs(lse.cpu().numpy().astype(np.float64) - ref_l)
-    assert (err <= 1e-3 + 16 * np.spacing(np.abs(ref_l).astype(np.float32))).all(), err.max()
-    # with scores in the thousands the softmax is nearly one-hot and near-ties between two keys
-    # flip on the bf16 rounding of P: max-abs 4e-2 here (2e-2 is BASELINE.json's bar for N(0,1) inputs)
-    e = np.abs(out.float().cpu().numpy().astype(np.float64) - ref_o)
-    assert e.max() <= 4e-2 and e.mean() <= 2e-3, (case, e.max(), e.mean())
+    # With scores in the thousands the softmax is nearly one-hot, so |out| reaches max|v| ~ 4.7 and
+    # the bf16 steps no longer average out: P is rounded to bf16 before the PV product (relative
+    # 2^-9 per weight, while the row sum uses the unrounded weights) and out is rounded to bf16
+    # (half an ulp <= 2^-8 |out|): |err| <= 3 * 2^-9 |out| = 5.9e-3 |out| (DESIGN.md section 3,
+    # "tolerances"). Below |out| = 3.4 that is inside BASELINE.json's 2e-2, which stays the bar;
+    # above it the bound is elementwise. The exact-running-max kernels (variants 1 and 3) run on
+    # the same inputs against the same bound; lse keeps BASELINE.json's 1e-3 although its values
+    # reach 2600 here (fp32 spacing 2.4e-4).
+    tol = np.maximum(OUT_MAX, 3 * 2.0 ** -9 * np.abs(ref_o))
+    for variant in (2, 1, 3):            # 2: pair items + score bound (the big-problem path)
+        out, lse = run_fwd(sa, q, k, v, bits, blk, scale, variant=variant)
+        lerr = np.abs(lse.cpu().numpy().astype(np.float64) - ref_l)
+        assert lerr.max() <= LSE_ABS, (case, variant, "lse", lerr.max())
+        e = np.abs(out.float().cpu().numpy().astype(np.float64) - ref_o)
+        assert (e <= tol).all(), (case, variant, "out", float((e / tol).max()), float(e.max()))
+        assert e.mean() <= OUT_MEAN, (case, variant, e.mean())
 
 
 @pytest.mark.parametrize("variant", [0, 1, 2])
@@ -326,7 +404,7 @@ def test_c3_full_size_sampled_units(sa):
     # BASELINE.json configs[2]: Wan2.1-14B 480p shapes, per-head density U(0.05, 0.35)
     cfg = inputs.C3
     q, k, v, bits, bits_t = _full_size_inputs(sa, cfg)
-    _, _, dense = _sampled_unit_parity(sa, cfg, q, k, v, bits, bits_t, variant=0, n_heads=4)
+    _, _, dense = _sampled_unit_parity(sa, cfg, q, k, v, bits, bits_t, variant=0, n_heads=8)
     per_head = dense.reshape(cfg.H, -1).mean(axis=1)
     assert 0.04 < per_head.min() < 0.12 and 0.28 < per_head.max() < 0.36     # uneven heads
 
@@ -335,7 +413,7 @@ def test_c4_full_size_sampled_units(sa):
     # the configuration bench.py times (Wan2.1-14B 720p shapes), same launch path
     cfg = inputs.C4
     q, k, v, bits, bits_t = _full_size_inputs(sa, cfg)
-    _sampled_unit_parity(sa, cfg, q, k, v, bits, bits_t, variant=0, n_heads=4)
+    _sampled_unit_parity(sa, cfg, q, k, v, bits, bits_t, variant=0, n_heads=8)   # 8 heads x 8 rows
 
 
 def test_c4_closed_forms_every_row(sa):
@@ -391,6 +469,30 @@ def test_c5_adversarial_and_sparse_sweep_sampled_units(sa):
                              force_diag=True)
     bits = host_bits(bits_t)
     _sampled_unit_parity(sa, cfg, q, k, v, bits, bits_t, variant=0, n_heads=2)
+
+
+@pytest.mark.parametrize("density", [1.0, 0.5, 0.25, 0.125])
+def test_c5_density_sweep_masks_sampled_units(sa, density):
+    # BASELINE.json config 5: uniform per-head density at the C4 shapes, the masks bench.py's sweep
+    # times (mask seed 104). Density 1 is the paper's "fully dense setting": 591 key
+    # blocks accumulated per row, the longest run of the fixed-reference softmax. Units: rows 0 and
+    # NQB-1 (ragged diagonal block, padded query rows), heaviest, lightest and seeded-random rows.
+    H = 2 if density == 1.0 else 4
+    cfg = inputs.scaled(inputs.C4, H=H)
+    q, k, v, bits, bits_t = _full_size_inputs(sa, cfg, uniform_density=density, mask_seed=104)
+    dense = oracle.unpack_mask(bits, cfg.NKB)
+    assert abs(dense.mean() - density) < 1e-3
+    units = inputs.sample_units(dense.sum(axis=2), seed=104, n_heads=2,
+                                n_random_rows=2 if density == 1.0 else 4)
+    assert {0, cfg.NQB - 1} <= set(units[:, 2].tolist())
+    ref_o, ref_l = oracle.attn_units(inputs.as_u16(q), inputs.as_u16(k), inputs.as_u16(v), bits,
+                                     units, cfg.Bq, cfg.Bk, cfg.scale, n_valid=cfg.n_valid)
+    out, lse = sa.sa_block_sparse_attn_fwd_ex(q.cuda(), k.cuda(), v.cuda(), bits_t, cfg.Bq, cfg.Bk,
+                                              cfg.scale, n_valid=cfg.n_valid)
+    torch.cuda.synchronize()
+    got_o = torch.stack([out[b, h, u * cfg.Bq:(u + 1) * cfg.Bq] for b, h, u in units.tolist()])
+    got_l = torch.stack([lse[b, h, u * cfg.Bq:(u + 1) * cfg.Bq] for b, h, u in units.tolist()])
+    check_out(got_o, got_l, ref_o, ref_l, f"C5 density {density}")
 
 
 def test_next1_262144_tokens_sampled_units(sa):
