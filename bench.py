@@ -87,30 +87,54 @@ def aggregate_replicas(active_blocks_local: int, flops_per_block: int, ms_local:
     return effective_tflops(int(blocks), flops_per_block, ms), ms, int(blocks)
 
 
-def parse_clock_csv(text: str) -> dict:
-    """Summarise `nvidia-smi --query-gpu=... --format=csv -lms` output sampled under load."""
-    sm, mx, reasons = [], [], set()
+def _clock_timestamp(field: str):
+    """nvidia-smi's `timestamp` field ("2026/11/05 01:23:45.678") as seconds since the epoch."""
+    import datetime
+    try:
+        return datetime.datetime.strptime(field.strip(), "%Y/%m/%d %H:%M:%S.%f").timestamp()
+    except ValueError:
+        return None
+
+
+def parse_clock_csv(text: str, t0: float | None = None, t1: float | None = None) -> dict:
+    """Summarise `nvidia-smi --query-gpu=... --format=csv -lms` output sampled under load. Lines may
+    start with a `timestamp` field; with t0/t1 (epoch seconds) only the samples taken inside
+    [t0, t1] count."""
+    sm, mx, pw, reasons = [], [], [], set()
     names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
     for line in text.splitlines():
         parts = [p.strip() for p in line.split(",")]
+        ts = None
+        if parts and "/" in parts[0]:
+            ts = _clock_timestamp(parts[0])
+            parts = parts[1:]
         if len(parts) < 9 or not parts[0].isdigit():
+            continue
+        if t0 is not None and (ts is None or ts < t0 or ts > t1):
             continue
         try:
             sm.append(float(parts[1].split()[0]))
             mx.append(float(parts[2].split()[0]))
         except ValueError:
             continue
+        try:
+            pw.append(float(parts[3].split()[0]))
+        except (ValueError, IndexError):
+            pass
         for name, val in zip(names, parts[5:9]):
             if val.lower() == "active":
                 reasons.add(name)
     if not sm:
         return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
-    return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons),
-            "samples": len(sm)}
+    out = {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons),
+           "samples": len(sm)}
+    if pw:
+        out["power_w_median"] = statistics.median(pw)
+    return out
 
 
 class ClockSampler:
-    QUERY = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+    QUERY = ("timestamp,index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
              "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
@@ -122,14 +146,14 @@ class ClockSampler:
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", "-i", str(self.gpu_index), "--query-gpu=" + self.QUERY,
-                 "--format=csv", "-lms", "50"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL,
+                 "--format=csv", "-lms", "20"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL,
                 text=True)
         except OSError:
             self.proc = None
         return self
 
-    def __exit__(self, *exc):
-        self.summary = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+    def stop(self):
+        self.text = ""
         if self.proc is not None:
             self.proc.terminate()
             try:
@@ -137,7 +161,16 @@ class ClockSampler:
             except subprocess.TimeoutExpired:
                 self.proc.kill()
                 out, _ = self.proc.communicate()
-            self.summary = parse_clock_csv(out or "")
+            self.text = out or ""
+            self.proc = None
+        self.summary = parse_clock_csv(self.text)
+
+    def window(self, t0: float, t1: float) -> dict:
+        """Summary of the samples taken between two time.time() stamps (after stop())."""
+        return parse_clock_csv(self.text, t0, t1)
+
+    def __exit__(self, *exc):
+        self.stop()
         return False
 
 
@@ -203,7 +236,11 @@ def run_reference(args, rank: int, world: int) -> int:
 
 
 # ------------------------------------------------------------------ our arm
-def run_seq_grid(sa, dev, stream, peaks, H: int, log):
+GRID_DEFAULT_N = (4096, 16384, 65536)          # the bounded grid of the default run (a few seconds)
+GRID_DEFAULT_DENSITY = (1.0, 0.25, 0.05)
+
+
+def run_seq_grid(sa, dev, stream, peaks, H: int, log, full: bool):
     """the paper's own kernel experiment (Fig. 5 caption
     PAPER.md:250) -- sequence length 1K..262K x density at block 128 -- plus a HunyuanVideo-shaped
     layer. The paper compares with FlashAttention-3; here density 1 of the same
@@ -213,7 +250,9 @@ def run_seq_grid(sa, dev, stream, peaks, H: int, log):
     import torch
     from paper_2606_23019_b200 import inputs
     rows = []
-    shapes = [inputs.seq_grid_config(N, H) for N in inputs.SEQ_GRID_N] + [inputs.HUNYUAN]
+    grid_n = inputs.SEQ_GRID_N if full else GRID_DEFAULT_N
+    densities = inputs.SEQ_GRID_DENSITY if full else GRID_DEFAULT_DENSITY
+    shapes = [inputs.seq_grid_config(N, H) for N in grid_n] + [inputs.HUNYUAN]
     for cfg in shapes:
         g = torch.Generator(device=dev).manual_seed(cfg.qkv_seed)
         q, k, v = [torch.randn((cfg.B, cfg.H, cfg.N, cfg.D), generator=g, device=dev,
@@ -225,12 +264,12 @@ def run_seq_grid(sa, dev, stream, peaks, H: int, log):
         scores_np, _ = inputs.iid_block_scores(cfg, 1.0)
         scores = torch.from_numpy(scores_np).to(dev)
         t_dense = None
-        for d in inputs.SEQ_GRID_DENSITY:
+        for d in densities:
             dens_t = torch.full((cfg.H,), d, dtype=torch.float32, device=dev)
             bits = sa.sa_pack_mask(scores, dens_t, True)
             torch.cuda.synchronize()
             nb = popcount_total(bits.cpu().numpy().view(np.uint32)) * cfg.B
-            reps = 3 if cfg.N >= 65536 and d >= 0.5 else 7
+            reps = 3 if cfg.N >= 65536 and d >= 0.5 else (7 if full else 5)
             for _ in range(2):
                 sa.sa_block_sparse_attn_fwd_ex(q, k, v, bits, cfg.Bq, cfg.Bk, cfg.scale,
                                                cfg.n_valid, out, lse, ws, stream)
@@ -245,6 +284,7 @@ def run_seq_grid(sa, dev, stream, peaks, H: int, log):
                 torch.cuda.synchronize()
                 ts.append(a.elapsed_time(b))
             med = statistics.median(ts)
+            n_launch = sa.sa_last_launch_count()
             # the static-mask form: the work list of the previous call is reused
             ts_r = []
             for _ in range(reps):
@@ -262,6 +302,7 @@ def run_seq_grid(sa, dev, stream, peaks, H: int, log):
             tf = effective_tflops(nb, cfg.flops_per_block(), med)
             rows.append({"shape": cfg.name, "N": cfg.N, "H": cfg.H, "density": round(dens, 5),
                          "ms_median": round(med, 4), "ms_median_reuse": round(med_reuse, 4),
+                         "launches_per_call": n_launch,
                          "tflops": round(tf, 1),
                          "frac_of_peak": round(tf / peaks["bf16_tflops"], 4),
                          "speedup_vs_density1": round(t_dense / med, 3),
@@ -382,24 +423,33 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> int:
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- device-resident leg
+    # ---- device-resident leg. The clock sampler starts before the warm-up (>= 0.5 s before the timed
+    # loop) and runs until the sweep is over; the timed loop's own samples are reported separately.
+    clk = ClockSampler(local_rank)
+    clk.__enter__()
+    t_sampler = time.time()
     for _ in range(args.warmup):
         step()
     barrier()
     active_blocks = popcount_total(bits.cpu().numpy().view(np.uint32)) * cfg.B
     row_pop = np.unpackbits(bits.cpu().numpy().view(np.uint8), axis=-1).reshape(
         cfg.H, cfg.NQB, -1).sum(axis=2)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    time.sleep(max(0.0, 0.5 - (time.time() - t_sampler)))
+    for _ in range(2):                       # two more untimed steps after the host-side pause
+        step()
+    barrier()
     sa.sa_profile_enable(args.steps)
     launches[0] = 0
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    with ClockSampler(local_rank) as clk:
-        barrier()
-        e0.record(stream)
-        for _ in range(args.steps):
-            step()
-        e1.record(stream)
-        barrier()
+    t_loop0 = time.time()
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    barrier()
+    t_loop1 = time.time()
     ms_local = e0.elapsed_time(e1) / args.steps
+    path_fixed, path_exact = sa.sa_fwd_softmax_path_counts(fwd_ws, stream)
     kernel_ms = sa.sa_profile_collect(args.steps)
     sa.sa_profile_enable(0)
     gpu_launches = launches[0]
@@ -488,12 +538,48 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> int:
             log(f"[bench] sweep {name}: density {dens:.4f} {med:.3f} ms {tf:.1f} TFLOP/s "
                 f"speedup {t_dense / med:.2f} (ideal {1 / dens:.2f})")
 
+    # ---- the same kernel on inputs whose Cauchy-Schwarz score bound is loose (q x 8, k x 4: real
+    # q/k with large norms, e.g. QK-norm gains): every row then keeps the exact running max with the
+    # lazy rescale instead of the fixed reference point the N(0,1) inputs above allow
+    loose = None
+    if rank == 0 and not args.no_sweep:
+        q8, k4 = (q.float() * 8).to(torch.bfloat16), (k.float() * 4).to(torch.bfloat16)
+        loose = []
+        for name, s_t, d_t in (("C4 mask", scores, density), cases[0]):
+            sa.sa_pack_mask(s_t.to(dev), d_t.to(dev), True, bits_s, pack_ws, stream)
+            torch.cuda.synchronize()
+            nb = popcount_total(bits_s.cpu().numpy().view(np.uint32)) * cfg.B
+            ts = []
+            for i in range(5):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                sa.sa_block_sparse_attn_fwd_ex(q8, k4, v, bits_s, cfg.Bq, cfg.Bk, cfg.scale, cfg.n_valid,
+                                               out, lse, fwd_ws, stream)
+                b.record(stream)
+                torch.cuda.synchronize()
+                if i >= 2:
+                    ts.append(a.elapsed_time(b))
+            med = statistics.median(ts)
+            fx, ex = sa.sa_fwd_softmax_path_counts(fwd_ws, stream)
+            tf = effective_tflops(nb, fpb, med)
+            loose.append({"case": "density 1" if name == "1" else name, "inputs": "q x 8, k x 4",
+                          "ms_median": round(med, 4), "tflops": round(tf, 1),
+                          "frac_of_peak": round(tf / peaks["bf16_tflops"], 4),
+                          "warp_items_fixed_reference": fx, "warp_items_exact_max": ex})
+            log(f"[bench] loose score bound, {name}: {med:.3f} ms {tf:.1f} TFLOP/s "
+                f"(softmax path: {fx} fixed / {ex} exact warp-items)")
+        del q8, k4
+    clk.stop()
+    clocks = dict(clk.summary)
+    clocks["window"] = "warm-up, timed loop, e2e leg, density sweep"
+    clocks["timed_loop"] = clk.window(t_loop0, t_loop1)
+
     seq_grid = None
-    if rank == 0 and args.seqlen_grid:
-        seq_grid = run_seq_grid(sa, dev, stream, peaks, args.grid_heads, log)
+    if rank == 0 and not args.no_grid:
+        seq_grid = run_seq_grid(sa, dev, stream, peaks, args.grid_heads, log, full=args.seqlen_grid)
 
     west = None
-    if rank == 0 and args.west:
+    if rank == 0 and not args.no_west:
         west = run_west_offline(sa, dev, stream, peaks, log)
 
     # ---- pack-mask kernel group on its own (HBM/ALU-bound; not the dominant kernel)
@@ -611,8 +697,10 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> int:
                     "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "api": "sa_hot_path_host", "matches_device_leg": same},
             "gpu_launches": gpu_launches,
-            "clocks": {"sm_mhz": clk.summary["sm_mhz"], "sm_max_mhz": clk.summary["sm_max_mhz"],
-                       "reasons": clk.summary["reasons"], "samples": clk.summary["samples"]},
+            "clocks": clocks,
+            "softmax_path": {"warp_items_fixed_reference": path_fixed, "warp_items_exact_max": path_exact,
+                             "note": "(softmax warp, work item) counts of the last timed step"},
+            "loose_score_bound": loose,
             "roofline": {
                 "kernel": "fwd_tcgen05_kernel", "bound": "tensor", "achieved": achieved,
                 "peak": peaks["bf16_tflops"], "unit": "TFLOP/s",
@@ -656,12 +744,14 @@ def main() -> int:
     ap.add_argument("--ref-rows-per-head", type=int, default=8)
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--seqlen-grid", action="store_true",
-                    help="also time the sequence-length x density grid (1K..262K tokens) and a "
-                         "HunyuanVideo-shaped layer; off by default to keep the default run short")
+                    help="time the FULL sequence-length x density grid (1K..262K tokens x 5 densities) "
+                         "instead of the bounded default (4K, 16K, 64K x {1, 0.25, 0.05}); the "
+                         "HunyuanVideo-shaped layer is in both")
+    ap.add_argument("--no-grid", action="store_true")
     ap.add_argument("--grid-heads", type=int, default=12)
-    ap.add_argument("--west", action="store_true",
-                    help="also time the offline per-sample steps (block significance, threshold-map "
-                         "update, fidelity) at Wan2.1-14B 480p shapes")
+    ap.add_argument("--no-west", action="store_true",
+                    help="skip the offline per-sample steps (block significance, threshold-map update, "
+                         "fidelity) at Wan2.1-14B 480p shapes")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

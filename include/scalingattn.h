@@ -226,6 +226,14 @@ SA_API sa_status sa_enumerate_active_blocks(const uint32_t* mask_bits, int H, in
 SA_API sa_status sa_set_fwd_variant(int variant);
 SA_API int sa_get_fwd_variant(void);
 
+/* Which softmax path the last forward call that used `workspace` took (tcgen05 kernel only; see
+ * DESIGN.md K1): per (softmax warp, work item) with at least one key block, *fixed_host counts those
+ * that fixed the reference point at the Cauchy-Schwarz score bound for the whole item and *exact_host
+ * those that kept the exact running max (bound too loose for the row norms at hand, or no key-norm
+ * pass on a small problem). Synchronises `stream`. Host pointers. */
+SA_API sa_status sa_fwd_softmax_path_counts(const void* workspace, long long* fixed_host,
+                                            long long* exact_host, void* stream);
+
 /* Debug hook: sa_block_sparse_attn_fwd_ex on a build of the (128,128,128) tcgen05 kernel that also
  * records its walk, so that the union walk of a work item (Alg. 2 re-expressed over the OR of two
  * bit-rows), the numbering of (tile, key block) units and the 64-word window reload can be checked

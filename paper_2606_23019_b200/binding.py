@@ -70,6 +70,8 @@ def load_library() -> C.CDLL:
                                                 fp, vp, sz, vp]
     lib.sa_block_sparse_attn_fwd_reuse.restype = ip
     lib.sa_block_sparse_attn_fwd_reuse.argtypes = lib.sa_block_sparse_attn_fwd_ex.argtypes
+    lib.sa_fwd_softmax_path_counts.restype = ip
+    lib.sa_fwd_softmax_path_counts.argtypes = [vp, vp, vp, vp]
     lib.sa_debug_fwd_walk_log_bytes.restype = sz
     lib.sa_debug_fwd_walk_log_bytes.argtypes = [ip] * 5
     lib.sa_debug_fwd_walk.restype = ip
@@ -285,6 +287,15 @@ def sa_block_sparse_attn_fwd_ex(q, k, v, mask_bits, Bq: int, Bk: int, scale: flo
                                            _ptr(lse), B, H, N, n_valid, D, Bq, Bk, float(scale),
                                            _ptr(workspace), workspace.numel(), _stream(stream)))
     return out, lse
+
+
+def sa_fwd_softmax_path_counts(workspace, stream=None):
+    """(fixed, exact): (softmax warp, work item) counts of the last tcgen05 forward call on `workspace`
+    by softmax path (fixed Cauchy-Schwarz reference point / exact running max)."""
+    a, b = C.c_longlong(0), C.c_longlong(0)
+    _check(load_library().sa_fwd_softmax_path_counts(_ptr(workspace), C.addressof(a), C.addressof(b),
+                                                     _stream(stream)))
+    return a.value, b.value
 
 
 def sa_debug_fwd_walk(q, k, v, mask_bits, Bq: int, Bk: int, scale: float, n_valid=None, stream=None):

@@ -302,6 +302,7 @@ static sa_status fwd_ex_impl(const void* q, const void* k, const void* v, const 
   p.items = w.items;
   p.n_items_dev = w.n_items;
   p.counter = w.cursor;
+  p.stats = w.stats;
   p.walk_log = walk_log;
   const int variant = walk_log ? 2 : g_variant.load(std::memory_order_relaxed);   // the walk log is the pair path's
   const bool fast = (variant != 1 && D == 128);
@@ -594,6 +595,21 @@ sa_status sa_enumerate_active_blocks(const uint32_t* mask_bits, int H, int NQB, 
   cudaError_t e = sa::launch_enumerate(mask_bits, H, NQB, NKB, idx, cnt,
                                        static_cast<cudaStream_t>(stream));
   if (e != cudaSuccess) return cuda_fail(e, "sa_enumerate_active_blocks launch");
+  return SA_OK;
+}
+
+sa_status sa_fwd_softmax_path_counts(const void* workspace, long long* fixed_host, long long* exact_host,
+                                     void* stream) {
+  if (!workspace || !fixed_host || !exact_host)
+    return fail(SA_ERR_INVALID_ARG, "sa_fwd_softmax_path_counts: null pointer");
+  int32_t c[2] = {0, 0};
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  cudaError_t e = cudaMemcpyAsync(c, static_cast<const int32_t*>(workspace) + 2, sizeof c,
+                                  cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) return cuda_fail(e, "sa_fwd_softmax_path_counts");
+  *fixed_host = c[0];
+  *exact_host = c[1];
   return SA_OK;
 }
 

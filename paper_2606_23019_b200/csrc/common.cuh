@@ -66,12 +66,15 @@ struct FwdParams {
   const float* kmax2;         // [B*H] max |k|^2 over the valid keys (tcgen05 kernel only)
   int n_items;                // host-side count: exact for single-row items, an upper bound for pairs
   int rows_per_item;          // query blocks per work item: 2 (a pair shares its K/V tiles) or 1
+  int32_t* stats;             // [2] (warp, item) counts by softmax path: fixed reference point / exact
+                              // running max (zeroed by the pre-pass; tcgen05 kernel only)
   int32_t* walk_log;          // sa_debug_fwd_walk only (else null): see WalkLog in fwd_tcgen05.cu
 };
 
 // Workspace layout for the forward pass (int32 words):
 //   [0]                  scheduler cursor
 //   [1]                  number of work items
+//   [2], [3]             (warp, item) counts of the last tcgen05 call by softmax path (fixed / exact)
 //   [16 .. 16+BH)        per-(b,h) total cost (active tiles)
 //   [.. + BH)            per-(b,h) number of items
 //   [.. + BH)            fp32: per (b,h) max over the valid keys of |k|^2
@@ -80,6 +83,7 @@ struct FwdParams {
 struct FwdWorkspace {
   int32_t* cursor;
   int32_t* n_items;
+  int32_t* stats;
   int32_t* head_cost;
   int32_t* head_count;
   float* kmax2;               // [B*H] max over valid keys of |k|^2

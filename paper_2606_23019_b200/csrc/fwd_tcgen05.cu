@@ -563,6 +563,7 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
   uint32_t nmine = 0;                    // this tile's units so far (barrier selection: every phase
                                          // of s_full[t][.] is consumed in order, none is skipped)
   int sched_n = 0;
+  uint32_t n_fixed = 0, n_exact = 0;     // items of this warp by softmax path (p.stats)
 #ifdef SA_TRACE
   uint32_t tr_acc[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, tr_last = clock(), tr_n = 0, tr_items = 0;
 #define SA_TR(i) { const uint32_t now_ = clock(); tr_acc[i] += now_ - tr_last; tr_last = now_; if (i == 4) ++tr_n; }
@@ -722,6 +723,8 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
           // scores (the real maximum over the item is at least this block's), and never exceeds 1
           fixed = __all_sync(0xFFFFFFFFu, m_run > -INFINITY && bound <= m_run + kBoundSlack);
           if (fixed) m_run = bound;
+          n_fixed += fixed ? 1u : 0u;
+          n_exact += fixed ? 0u : 1u;
         }
         }
         const float m_use = (m_run == -INFINITY) ? 0.f : m_run;
@@ -804,6 +807,10 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
       for (int i = 0; i < 16; ++i) orow[i] = z;
       p.lse[grow] = -INFINITY;
     }
+  }
+  if (p.stats != nullptr && lane == 0) {
+    atomicAdd(p.stats, static_cast<int32_t>(n_fixed));
+    atomicAdd(p.stats + 1, static_cast<int32_t>(n_exact));
   }
 #ifdef SA_TRACE
   if (lane == 0 && blockIdx.x < 2 && quarter == 0)

@@ -23,7 +23,7 @@ namespace sa {
 
 size_t fwd_workspace_bytes(int B, int H, int NQB) {
   const size_t BH = static_cast<size_t>(B) * H;
-  const size_t words = 16 + 3 * BH + 4 * BH * static_cast<size_t>(NQB);   // two int2 arrays of BH*NQB records
+  const size_t words = 18 + 3 * BH + 4 * BH * static_cast<size_t>(NQB);   // two int2 arrays of BH*NQB records (+ alignment)
   return ((words * sizeof(int32_t) + 255) / 256) * 256;
 }
 
@@ -33,6 +33,7 @@ FwdWorkspace carve_fwd_workspace(void* ws, int B, int H, int NQB) {
   FwdWorkspace w;
   w.cursor = p;
   w.n_items = p + 1;
+  w.stats = p + 2;
   w.head_cost = p + 16;
   w.head_count = w.head_cost + BH;
   w.kmax2 = reinterpret_cast<float*>(w.head_count + BH);
@@ -293,7 +294,8 @@ schedule_flatten_kernel(const int32_t* __restrict__ head_cost, const int32_t* __
         items[s_start + pos] = make_int2(bh, rec.y);
       }
       if (first && threadIdx.x == 0) {
-        *cursor = 0;
+        cursor[0] = 0;
+        cursor[2] = cursor[3] = 0;    // softmax-path counters of the coming call
         *n_items = s_all;
       }
     }
@@ -328,6 +330,7 @@ cudaError_t launch_schedule(const FwdParams& p, const FwdWorkspace& w, int rpi, 
   if (reuse) {
     // the work list in the workspace is still valid (same mask): only reset what a call consumes
     e = cudaMemsetAsync(w.cursor, 0, sizeof(int32_t), st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(w.stats, 0, 2 * sizeof(int32_t), st);
     if (e == cudaSuccess && norms) e = cudaMemsetAsync(w.kmax2, 0, static_cast<size_t>(BH) * sizeof(float), st);
     if (e != cudaSuccess) return e;
   } else {

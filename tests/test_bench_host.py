@@ -37,6 +37,16 @@ def test_parse_clock_csv():
     assert s["samples"] == 3 and s["sm_mhz"] == 1410.0 and s["sm_max_mhz"] == 1965.0
     assert s["reasons"] == ["sw_power_cap"]
     assert bench.parse_clock_csv("garbage\n")["samples"] == 0
+    # timestamped form (what ClockSampler asks for) and a time window
+    import datetime
+    t0 = datetime.datetime(2026, 11, 5, 1, 2, 3).timestamp()
+    rows = "".join(
+        f"2026/11/05 01:02:0{3 + i}.500, 0, {1500 + 10 * i} MHz, 1965 MHz, {900 + i}.0 W, 0x4, Not Active, "
+        f"Not Active, Not Active, Active\n" for i in range(5))
+    s = bench.parse_clock_csv("timestamp, index, ...\n" + rows)
+    assert s["samples"] == 5 and s["sm_mhz"] == 1520.0 and s["power_w_median"] == 902.0
+    w = bench.parse_clock_csv(rows, t0 + 1.0, t0 + 3.0)         # samples at +1.5 and +2.5 s
+    assert w["samples"] == 2 and w["sm_mhz"] == 1515.0
 
 
 def test_load_peaks_has_measured_or_fallback():
