@@ -6,7 +6,6 @@ loaded, or a call returns a non-OK status, SAError is raised.
 """
 from __future__ import annotations
 
-import contextlib
 import ctypes as C
 import os
 
@@ -15,7 +14,6 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libscalingattn.so")
 _lib = None
-_null_ctx = contextlib.nullcontext
 
 SA_OK = 0
 
@@ -118,6 +116,17 @@ def _stream(stream) -> int:
     return stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
 
 
+def _scratch(nbytes: int, device, stream):
+    """A temporary device buffer for one call. The caching allocator ties a block to the stream that
+    was current when it was allocated; when the call runs on another stream the block is marked as
+    in use there (record_stream), so that it is not handed out again while the kernels are pending."""
+    t = torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=device)
+    if stream is not None:
+        s = stream if isinstance(stream, torch.cuda.Stream) else torch.cuda.ExternalStream(int(stream))
+        t.record_stream(s)
+    return t
+
+
 def sa_status_string(status: int) -> str:
     return load_library().sa_status_string(status).decode()
 
@@ -168,7 +177,7 @@ def sa_pack_mask(scores, density, force_diag: bool = True, mask_bits=None, works
         mask_bits = torch.empty((H, NQB, W), dtype=torch.int32, device=scores.device)
     need = lib.sa_pack_mask_workspace_bytes(H, NQB, NKB)
     if workspace is None:
-        workspace = torch.empty(need, dtype=torch.uint8, device=scores.device)
+        workspace = _scratch(need, scores.device, stream)
     _check(lib.sa_pack_mask(_ptr(scores), _ptr(density), _ptr(mask_bits), H, NQB, NKB,
                             int(bool(force_diag)), _ptr(workspace), workspace.numel(),
                             _stream(stream)))
@@ -219,7 +228,7 @@ def sa_threshold_map_update(sig, levels, tmap, workspace=None, stream=None):
     assert tmap.dtype == torch.float32 and tmap.is_contiguous() and tuple(tmap.shape) == (H, NQB, NKB)
     need = lib.sa_threshold_map_update_workspace_bytes(B, H, NQB, NKB)
     if workspace is None:
-        workspace = torch.empty(max(need, 256), dtype=torch.uint8, device=sig.device)
+        workspace = _scratch(need, sig.device, stream)
     _check(lib.sa_threshold_map_update(_ptr(sig), _ptr(levels), levels.numel(), _ptr(tmap), B, H, NQB,
                                        NKB, _ptr(workspace), workspace.numel(), _stream(stream)))
     return tmap
@@ -280,8 +289,10 @@ def sa_block_sparse_attn_fwd_ex(q, k, v, mask_bits, Bq: int, Bk: int, scale: flo
     if lse is None:
         lse = torch.empty((B, H, N), dtype=torch.float32, device=q.device)
     if workspace is None:
-        workspace = torch.empty(max(lib.sa_fwd_workspace_bytes(B, H, N, Bq), 256),
-                                dtype=torch.uint8, device=q.device)
+        if reuse_schedule:
+            raise ValueError("reuse_schedule=True needs the caller-owned workspace of the earlier call "
+                             "(a fresh workspace holds no work list)")
+        workspace = _scratch(lib.sa_fwd_workspace_bytes(B, H, N, Bq), q.device, stream)
     fn = lib.sa_block_sparse_attn_fwd_reuse if reuse_schedule else lib.sa_block_sparse_attn_fwd_ex
     _check(fn(_ptr(q), _ptr(k), _ptr(v), _ptr(mask_bits), _ptr(out),
                                            _ptr(lse), B, H, N, n_valid, D, Bq, Bk, float(scale),
@@ -307,11 +318,11 @@ def sa_debug_fwd_walk(q, k, v, mask_bits, Bq: int, Bk: int, scale: float, n_vali
     n_valid = N if n_valid is None else int(n_valid)
     out = torch.empty_like(q)
     lse = torch.empty((B, H, N), dtype=torch.float32, device=q.device)
-    with torch.cuda.stream(stream) if stream is not None else _null_ctx():
-        workspace = torch.empty(max(lib.sa_fwd_workspace_bytes(B, H, N, Bq), 256), dtype=torch.uint8,
-                                device=q.device)
-        log = torch.zeros(lib.sa_debug_fwd_walk_log_bytes(B, H, N, Bq, Bk) // 4, dtype=torch.int32,
-                          device=q.device)
+    workspace = _scratch(lib.sa_fwd_workspace_bytes(B, H, N, Bq), q.device, stream)
+    log = torch.zeros(lib.sa_debug_fwd_walk_log_bytes(B, H, N, Bq, Bk) // 4, dtype=torch.int32,
+                      device=q.device)
+    if stream is not None:      # the zero fill ran on the current stream
+        torch.cuda.current_stream().synchronize()
     _check(lib.sa_debug_fwd_walk(_ptr(q), _ptr(k), _ptr(v), _ptr(mask_bits), _ptr(out), _ptr(lse), B, H, N,
                                  n_valid, D, Bq, Bk, float(scale), _ptr(workspace), workspace.numel(),
                                  _ptr(log), log.numel() * 4, _stream(stream)))

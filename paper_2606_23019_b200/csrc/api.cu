@@ -83,15 +83,21 @@ void prof_free() {
   g_prof_n = 0;
 }
 
-// internal workspace of the short-signature call
+// Internal workspaces of the short-signature call, one per (device, stream): the workspace holds the
+// scheduler cursor and the work list, which a call rebuilds while an earlier call's persistent kernel
+// may still be consuming them -- safe only in stream order. Calls on the same stream are ordered by
+// the stream (the mutex is held across the enqueue, so two threads sharing a stream cannot interleave
+// their launches); calls on different streams get different buffers. Buffers are allocated and, when
+// they have to grow, freed in stream order (cudaMallocAsync / cudaFreeAsync on the caller's stream),
+// so a buffer is never released while work that uses it is pending.
+struct StreamWs {
+  int dev;
+  cudaStream_t stream;
+  void* ptr;
+  size_t bytes;
+};
 std::mutex g_ws_mu;
-void* g_ws = nullptr;
-size_t g_ws_bytes = 0;
-struct WsFree {
-  ~WsFree() {
-    if (g_ws) cudaFree(g_ws);
-  }
-} g_ws_free;
+std::vector<StreamWs> g_ws;
 
 // Copy engines for the host-buffer entry points: the q/k/v upload of head group g+1 and the out/lse
 // download of group g-1 overlap the forward pass of group g (PCIe is full duplex and the copy engines
@@ -112,7 +118,8 @@ struct PipeCtx {
   }
 };
 std::mutex g_pipe_mu;
-PipeCtx g_pipe;
+constexpr int kMaxPipeDevices = 64;
+PipeCtx g_pipes[kMaxPipeDevices];   // streams and events belong to a device: one context per ordinal
 constexpr int kPipeGroups = 8;     // head groups per batch entry (fewer when H is small)
 
 }  // namespace
@@ -179,10 +186,10 @@ sa_status sa_mask_from_threshold(const float* tmap, const float* p_star, uint32_
                 nbq, nbk, NQB, NKB);
   if (!aligned16(tmap) || !aligned16(mask_bits))
     return fail(SA_ERR_INVALID_ARG, "sa_mask_from_threshold: pointers must be 16-byte aligned");
-  if (nbq > 32768 || nbk > 32768 || NQB > 32768 || NKB > 32768 ||
+  if (H > 65535 || nbq > 32768 || nbk > 32768 || NQB > 32768 || NKB > 32768 ||
       static_cast<long long>(H) * NQB * ((NKB + 31) / 32) > 0x3FFFFFFFLL)
     return fail(SA_ERR_UNSUPPORTED,
-                "sa_mask_from_threshold: a grid side exceeds 32768 blocks or the mask 2^30 words");
+                "sa_mask_from_threshold: H > 65535, a grid side exceeds 32768 blocks or the mask 2^30 words");
   sa_status s = check_device();
   if (s != SA_OK) return s;
   cudaError_t e = sa::launch_mask_from_threshold(tmap, p_star, mask_bits, H, nbq, nbk, NQB, NKB,
@@ -388,24 +395,31 @@ sa_status sa_block_sparse_attn_fwd(const void* q, const void* k, const void* v,
                                    int N, int D, int Bq, int Bk, float scale, void* stream) {
   const size_t need = sa_fwd_workspace_bytes(B, H, N, Bq);
   if (need == 0) return fail(SA_ERR_INVALID_ARG, "sa_block_sparse_attn_fwd: bad sizes");
-  void* ws = nullptr;
-  {
-    std::lock_guard<std::mutex> lk(g_ws_mu);
-    if (g_ws_bytes < need) {
-      if (g_ws) {
-        cudaDeviceSynchronize();
-        cudaFree(g_ws);
-        g_ws = nullptr;
-        g_ws_bytes = 0;
-      }
-      cudaError_t e = cudaMalloc(&g_ws, need);
-      if (e != cudaSuccess) return cuda_fail(e, "cudaMalloc(internal workspace)");
-      g_ws_bytes = need;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  std::lock_guard<std::mutex> lk(g_ws_mu);          // held until the call's kernels are enqueued
+  StreamWs* slot = nullptr;
+  for (StreamWs& w : g_ws)
+    if (w.dev == dev && w.stream == st) slot = &w;
+  if (!slot) {
+    g_ws.push_back(StreamWs{dev, st, nullptr, 0});
+    slot = &g_ws.back();
+  }
+  if (slot->bytes < need) {
+    if (slot->ptr) {
+      e = cudaFreeAsync(slot->ptr, st);             // after the stream's pending work that uses it
+      if (e != cudaSuccess) return cuda_fail(e, "cudaFreeAsync(internal workspace)");
+      slot->ptr = nullptr;
+      slot->bytes = 0;
     }
-    ws = g_ws;
+    e = cudaMallocAsync(&slot->ptr, need, st);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaMallocAsync(internal workspace)");
+    slot->bytes = need;
   }
   return sa_block_sparse_attn_fwd_ex(q, k, v, mask_bits, out, lse, B, H, N, N, D, Bq, Bk, scale,
-                                     ws, need, stream);
+                                     slot->ptr, need, stream);
 }
 
 // q, k, v up / forward / out, lse down, pipelined over head groups (see PipeCtx). The mask is already
@@ -418,8 +432,13 @@ static sa_status pipelined_fwd_host(const void* q_host, const void* k_host, cons
                                     cudaStream_t st, int* launches) {
   const int groups = H < kPipeGroups ? H : kPipeGroups;
   const int n_chunks = B * groups;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess || dev < 0 || dev >= kMaxPipeDevices)
+    return cuda_fail(e != cudaSuccess ? e : cudaErrorInvalidDevice, "cudaGetDevice");
   std::lock_guard<std::mutex> lk(g_pipe_mu);
-  cudaError_t e = g_pipe.init(2 * static_cast<size_t>(n_chunks) + 2);
+  PipeCtx& g_pipe = g_pipes[dev];
+  e = g_pipe.init(2 * static_cast<size_t>(n_chunks) + 2);
   if (e != cudaSuccess) return cuda_fail(e, "copy pipeline setup");
   cudaEvent_t ev_start = g_pipe.ev[0], ev_end = g_pipe.ev[1];
   if ((e = cudaEventRecord(ev_start, st)) != cudaSuccess ||

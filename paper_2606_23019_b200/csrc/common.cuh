@@ -96,7 +96,7 @@ FwdWorkspace carve_fwd_workspace(void* ws, int B, int H, int NQB);
 // per-device state (device.cu): SM count of the current device; dynamic shared-memory opt-in of a
 // kernel, set once per (device, kernel)
 enum SmemKernel { kSmemFwdTcgen05 = 0, kSmemFwdTcgen05Log, kSmemSigTcgen05, kSmemScheduleItems, kSmemFwdMmaSync64,
-                  kSmemFwdMmaSync128, kNumSmemKernels };
+                  kSmemFwdMmaSync128, kSmemMaskFromThreshold, kNumSmemKernels };
 cudaError_t device_sm_count(int* n_sm);
 cudaError_t ensure_dynamic_smem(SmemKernel id, const void* func, int bytes);
 

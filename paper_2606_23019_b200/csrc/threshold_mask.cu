@@ -10,56 +10,81 @@
 // active (readings P14-P16), so no floating-point interpolation is needed: with
 // x = u * nbq / NQB the cell a0 = floor(x) always has positive weight and a0 + 1 has one iff
 // (u * nbq) % NQB != 0 (clamped at the last cell); likewise along v. All of it is integer work, so
-// the result is bit-exact by construction. One warp produces one 32-bit mask word per step with
-// __ballot_sync; lanes read consecutive key blocks (coalesced). HBM/L2-bound streaming: the map
-// is read once (up to 4 neighbouring cells per target block, which share cache lines).
+// the result is bit-exact by construction.
+//
+// Layout of the work (HBM/L2-bound streaming; the map is 10.5 MB and the mask 1.8 MB at H = 40,
+// 256 x 256 -> 591 x 591): a CTA takes 32 target rows of one head. The column map v -> (b0, second
+// column?) does not depend on the row: it is computed once per CTA into shared memory (one integer
+// division per target column per CTA instead of two per mask bit). A warp then takes a target row:
+// it reads the row's one or two base rows with coalesced loads, compares with p* and ORs them into
+// a packed bit-row in shared memory (__ballot_sync), and every target bit is two shared-memory
+// lookups into that bit-row. Mask words are written 32 at a time (one coalesced store per 32 words).
 #include "common.cuh"
 
 namespace sa {
 namespace {
 
 constexpr int kThreads = 256;
+constexpr int kWarps = kThreads / 32;
+constexpr int kRowsPerBlock = 32;
 
-// one warp per bit-row (h, u): the two base rows are fixed for the row; 32-bit index arithmetic
-// (the host side bounds the sizes so that u * nbq and v * nbk stay below 2^31). Measured at the
-// 480p -> 720p shape (H = 40): 49 us per call; one warp per mask WORD was slower (90 us: the
-// per-word index divisions dominate), so the row form stays.
+// dynamic shared memory: uint16 colmap[NKB] (b0 | second column << 15), then per warp nbw =
+// ceil(nbk / 32) words of the ORed base bit-row
 __global__ void __launch_bounds__(kThreads)
 mask_from_threshold_kernel(const float* __restrict__ tmap, const float* __restrict__ p_star,
-                           uint32_t* __restrict__ mask_bits, int H, int nbq, int nbk, int NQB,
-                           int NKB, int W, int force_diag) {
-  const int lane = threadIdx.x & 31;
-  const int n_rows = H * NQB;            // < 2^31 (checked by the caller)
-  const int warp0 = (blockIdx.x * kThreads + threadIdx.x) >> 5;
-  const int n_warps = (gridDim.x * kThreads) >> 5;
-  for (int r = warp0; r < n_rows; r += n_warps) {
-    const int h = r / NQB, u = r - h * NQB;
-    const float p = __ldg(p_star + h);
+                           uint32_t* __restrict__ mask_bits, int nbq, int nbk, int NQB, int NKB, int W,
+                           int force_diag) {
+  extern __shared__ uint32_t s_dyn[];
+  const int nbw = (nbk + 31) / 32;
+  uint32_t* s_bits = s_dyn;                                          // [kWarps][nbw]
+  uint16_t* s_col = reinterpret_cast<uint16_t*>(s_dyn + kWarps * nbw);   // [NKB]
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int h = blockIdx.y;
+  for (int v = threadIdx.x; v < NKB; v += kThreads) {
+    const uint32_t yv = static_cast<uint32_t>(v) * static_cast<uint32_t>(nbk);   // < 2^31 (host check)
+    const uint32_t b0 = yv / static_cast<uint32_t>(NKB);
+    const bool two = (yv - b0 * static_cast<uint32_t>(NKB) != 0u) && (b0 + 1u < static_cast<uint32_t>(nbk));
+    s_col[v] = static_cast<uint16_t>(b0 | (two ? 0x8000u : 0u));
+  }
+  __syncthreads();
+  const float p = __ldg(p_star + h);
+  uint32_t* my_bits = s_bits + warp * nbw;
+  const int u_end = min((blockIdx.x + 1) * kRowsPerBlock, NQB);
+  for (int u = blockIdx.x * kRowsPerBlock + warp; u < u_end; u += kWarps) {
     const uint32_t xu = static_cast<uint32_t>(u) * static_cast<uint32_t>(nbq);
-    const int a0 = static_cast<int>(xu / static_cast<uint32_t>(NQB));
-    const bool two_rows = (xu % static_cast<uint32_t>(NQB) != 0u) && (a0 + 1 < nbq);
+    const uint32_t a0 = xu / static_cast<uint32_t>(NQB);
+    const bool two_rows = (xu - a0 * static_cast<uint32_t>(NQB) != 0u) && (a0 + 1u < static_cast<uint32_t>(nbq));
     const float* row0 = tmap + (static_cast<size_t>(h) * nbq + a0) * nbk;
     const float* row1 = two_rows ? row0 + nbk : row0;
-    uint32_t* dst = mask_bits + static_cast<size_t>(r) * W;
-#pragma unroll 4
-    for (int wv = 0; wv < W; ++wv) {
-      const int v = wv * 32 + lane;
+    // active base cells of the row's one or two base rows, ORed, as packed bits
+    for (int wb = 0; wb < nbw; ++wb) {
+      const int b = wb * 32 + lane;
       bool on = false;
-      if (v < NKB) {
-        const uint32_t yv = static_cast<uint32_t>(v) * static_cast<uint32_t>(nbk);
-        const int b0 = static_cast<int>(yv / static_cast<uint32_t>(NKB));
-        const bool two_cols = (yv % static_cast<uint32_t>(NKB) != 0u) && (b0 + 1 < nbk);
-        on = __ldg(row0 + b0) <= p;
-        if (two_cols) on = on || __ldg(row0 + b0 + 1) <= p;
-        if (two_rows) {
-          on = on || __ldg(row1 + b0) <= p;
-          if (two_cols) on = on || __ldg(row1 + b0 + 1) <= p;
-        }
-        if (force_diag && u == v) on = true;
-      }
-      const uint32_t bits = __ballot_sync(0xFFFFFFFFu, on);
-      if (lane == 0) dst[wv] = bits;
+      if (b < nbk) on = (__ldg(row0 + b) <= p) || (__ldg(row1 + b) <= p);
+      const uint32_t x = __ballot_sync(0xFFFFFFFFu, on);
+      if (lane == 0) my_bits[wb] = x;
     }
+    __syncwarp();
+    uint32_t* dst = mask_bits + (static_cast<size_t>(h) * NQB + u) * W;
+    for (int w0 = 0; w0 < W; w0 += 32) {
+      uint32_t mine = 0u;
+      const int wn = min(32, W - w0);
+      for (int i = 0; i < wn; ++i) {
+        const int v = (w0 + i) * 32 + lane;
+        bool on = false;
+        if (v < NKB) {
+          const uint32_t c = s_col[v];
+          const uint32_t b0 = c & 0x7FFFu;
+          on = (my_bits[b0 >> 5] >> (b0 & 31u)) & 1u;
+          if (c & 0x8000u) on = on || ((my_bits[(b0 + 1u) >> 5] >> ((b0 + 1u) & 31u)) & 1u);
+          if (force_diag && u == v) on = true;
+        }
+        const uint32_t x = __ballot_sync(0xFFFFFFFFu, on);
+        if (lane == i) mine = x;
+      }
+      if (lane < wn) dst[w0 + lane] = mine;
+    }
+    __syncwarp();                                  // my_bits is rewritten for the warp's next row
   }
 }
 
@@ -69,13 +94,15 @@ cudaError_t launch_mask_from_threshold(const float* tmap, const float* p_star, u
                                        int H, int nbq, int nbk, int NQB, int NKB, int force_diag,
                                        cudaStream_t st) {
   const int W = (NKB + 31) / 32;
-  const long long n_rows = static_cast<long long>(H) * NQB;
-  long long blocks = (n_rows * 32 + kThreads - 1) / kThreads;
-  const long long cap = 148LL * 8 * 4;     // grid-stride beyond 4 waves of 8 resident CTAs per SM
-  if (blocks > cap) blocks = cap;
-  if (blocks < 1) blocks = 1;
-  mask_from_threshold_kernel<<<static_cast<unsigned>(blocks), kThreads, 0, st>>>(
-      tmap, p_star, mask_bits, H, nbq, nbk, NQB, NKB, W, force_diag);
+  const size_t smem = static_cast<size_t>(kWarps) * ((nbk + 31) / 32) * 4 + static_cast<size_t>(NKB) * 2;
+  if (smem > 48 * 1024) {
+    cudaError_t e = ensure_dynamic_smem(kSmemMaskFromThreshold,
+                                        reinterpret_cast<const void*>(mask_from_threshold_kernel), 100 * 1024);
+    if (e != cudaSuccess) return e;
+  }
+  const dim3 grid((NQB + kRowsPerBlock - 1) / kRowsPerBlock, H);
+  mask_from_threshold_kernel<<<grid, kThreads, smem, st>>>(tmap, p_star, mask_bits, nbq, nbk, NQB, NKB, W,
+                                                          force_diag);
   return cudaGetLastError();
 }
 

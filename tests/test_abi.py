@@ -116,6 +116,28 @@ def test_offline_entry_points_validation(lib):
     assert fid(16, 16, 16, 0, 1, 2, 1024, 16, None, None) == INVALID
 
 
+def test_binding_refuses_schedule_reuse_without_workspace(lib):
+    # a fresh workspace holds no work list: the binding must not hand one to the _reuse entry point
+    import torch
+    from paper_2606_23019_b200 import binding
+    q = torch.zeros((1, 1, 128, 128), dtype=torch.bfloat16)
+    bits = torch.zeros((1, 1, 1), dtype=torch.int32)
+    with pytest.raises(ValueError):
+        binding.sa_block_sparse_attn_fwd_ex(q, q, q, bits, 128, 128, 0.1, reuse_schedule=True)
+
+
+def test_debug_and_stats_entry_points_validation(lib):
+    lib.sa_debug_fwd_walk_log_bytes.restype = C.c_size_t
+    assert lib.sa_debug_fwd_walk_log_bytes(1, 2, 1024, 128, 128) == (3 * 16 + 3 * 16 * 8) * 4
+    assert lib.sa_debug_fwd_walk_log_bytes(1, 2, 1000, 128, 128) == 0
+    # (64,64,64) has no walk-recording kernel; a short log is refused before any CUDA call
+    assert lib.sa_debug_fwd_walk(16, 16, 16, 16, 16, 16, 1, 2, 1024, 1024, 64, 64, 64, 0.125, 16, 1 << 20,
+                                 16, 1 << 20, None) == 2
+    assert lib.sa_debug_fwd_walk(16, 16, 16, 16, 16, 16, 1, 2, 1024, 1024, 128, 128, 128, 0.125, 16, 1 << 20,
+                                 16, 64, None) == 4
+    assert lib.sa_fwd_softmax_path_counts(None, None, None, None) == 1
+
+
 def test_product_does_not_import_oracle():
     # the product path must not route through the oracle (or any CPU fallback)
     pkg = os.path.join(ROOT, "paper_2606_23019_b200")

@@ -738,6 +738,27 @@ def test_threshold_map_update_matches_alg1(sa, B, H, NQB, NKB):
     assert np.array_equal(got.astype(np.float64), ref), np.abs(got - ref).max()
 
 
+def test_threshold_map_update_many_ties_across_sort_tiles(sa):
+    # "Sort S" (Alg. 1 l.12) is a hand-written stable radix sort working in tiles of 4096 elements:
+    # 100 x 90 = 9000 blocks per head span three tiles with a ragged last one, and significances
+    # quantised to 1/64 put long runs of equal keys across the tile and warp boundaries, so any
+    # slip in the stable ranks shows up as a wrong level (ties rank by flat index, P19).
+    # All sums are exact in fp64 here (multiples of 1/64), so the levels must agree exactly.
+    B, H, NQB, NKB = 2, 2, 100, 90
+    rng = np.random.Generator(np.random.PCG64(4096))
+    sig = (np.floor(rng.random((B, H, NQB, NKB)) ** 4 * 64) / 64).astype(np.float32)
+    sig[0, 1] = 0.25                                            # one head: every key equal
+    levels = (np.arange(1, 33) / 32.0).astype(np.float32)
+    ref = np.ones((H, NQB, NKB), dtype=np.float64)
+    for b in range(B):
+        for h in range(H):
+            ref[h] = oracle_west.threshold_map_update(ref[h], sig[b, h], levels)
+    tmap = torch.ones((H, NQB, NKB), dtype=torch.float32, device="cuda")
+    sa.sa_threshold_map_update(torch.from_numpy(sig).cuda(), torch.from_numpy(levels).cuda(), tmap)
+    torch.cuda.synchronize()
+    assert np.array_equal(tmap.cpu().numpy().astype(np.float64), ref)
+
+
 def test_west_pipeline_dense_lse_to_mask(sa):
     # the paper's offline path end to end on synthetic q, k (no calibration prompts here): dense
     # forward -> lse -> Eq. 1 -> Alg. 1 l.12-17 -> M_p = 1(T <= p) -> sparse forward -> fidelity
@@ -842,6 +863,41 @@ def test_schedule_reuse_is_bit_identical(sa, D, blk):
         torch.cuda.synchronize()
         assert torch.equal(full[0], again[0]) and torch.equal(full[1], again[1])
     assert sa.sa_last_launch_count() == 1     # the attention kernel only (small problem: no key-norm pass)
+
+
+def test_short_signature_call_on_two_streams(sa):
+    # sa_block_sparse_attn_fwd keeps its internal workspace (cursor, work list) per stream: calls
+    # issued back to back on two streams, with different masks and sizes, must not share it
+    D, blk = 128, 128
+    cases = []
+    for seed, H, nblk in ((21, 3, 12), (22, 2, 20)):
+        q, k, v, m = _small_case(D, blk, H, nblk, seed=seed, p=0.5)
+        m[:, np.arange(nblk), np.arange(nblk)] = True
+        bits = dev_bits(oracle.pack_bool(m))
+        cases.append((q.cuda(), k.cuda(), v.cuda(), bits))
+    scale = float(np.float32(1 / math.sqrt(D)))
+    want = [sa.sa_block_sparse_attn_fwd_ex(q, k, v, b, blk, blk, scale) for q, k, v, b in cases]
+    torch.cuda.synchronize()
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    reps = 6                                   # outputs of every call stay alive until the check
+    outs = [[(torch.empty_like(q), torch.empty(q.shape[:3], dtype=torch.float32, device="cuda"))
+             for q, _, _, _ in cases] for _ in range(reps)]
+    torch.cuda.synchronize()
+    for rep in range(reps):                    # interleaved, no synchronisation in between
+        for i, (q, k, v, b) in enumerate(cases):
+            sa.sa_block_sparse_attn_fwd(q, k, v, b, blk, blk, scale, out=outs[rep][i][0],
+                                        lse=outs[rep][i][1], stream=streams[i])
+    torch.cuda.synchronize()
+    for rep in range(reps):
+        for (o, l), (wo, wl) in zip(outs[rep], want):
+            assert torch.equal(o, wo) and torch.equal(l, wl)
+    # the same stream with a larger problem afterwards: the stream's buffer grows in stream order
+    q, k, v, m = _small_case(D, blk, 4, 40, seed=23, p=0.3)
+    bits = dev_bits(oracle.pack_bool(m))
+    wo, wl = sa.sa_block_sparse_attn_fwd_ex(q.cuda(), k.cuda(), v.cuda(), bits, blk, blk, scale)
+    o, l = sa.sa_block_sparse_attn_fwd(q.cuda(), k.cuda(), v.cuda(), bits, blk, blk, scale, stream=streams[0])
+    torch.cuda.synchronize()
+    assert torch.equal(o, wo) and torch.equal(l, wl)
 
 
 def test_cuda_library_is_the_path(sa):
