@@ -621,7 +621,7 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
           qn2 = fmaf(hi, hi, qn2);
         }
       }
-      bound = p.kmax2 ? c * sqrtf(qn2) * sqrtf(kmax2) : INFINITY;   // no bound: exact max
+      bound = (p.kmax2 && kmax2 >= 0.f) ? c * sqrtf(qn2) * sqrtf(kmax2) : INFINITY;   // no bound: exact max
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(smem_u32(&ctl->q_empty));   // this warp is done with the Q tiles

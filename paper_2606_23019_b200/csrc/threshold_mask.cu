@@ -57,12 +57,21 @@ mask_from_threshold_kernel(const float* __restrict__ tmap, const float* __restri
     const float* row0 = tmap + (static_cast<size_t>(h) * nbq + a0) * nbk;
     const float* row1 = two_rows ? row0 + nbk : row0;
     // active base cells of the row's one or two base rows, ORed, as packed bits
-    for (int wb = 0; wb < nbw; ++wb) {
-      const int b = wb * 32 + lane;
-      bool on = false;
-      if (b < nbk) on = (__ldg(row0 + b) <= p) || (__ldg(row1 + b) <= p);
-      const uint32_t x = __ballot_sync(0xFFFFFFFFu, on);
-      if (lane == 0) my_bits[wb] = x;
+    // (16 loads in flight per lane: the pass is latency-bound otherwise)
+    for (int wb0 = 0; wb0 < nbw; wb0 += 8) {
+      float x0[8], x1[8];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const int b = (wb0 + i) * 32 + lane;
+        const bool in = b < nbk;
+        x0[i] = in ? __ldg(row0 + b) : INFINITY;
+        x1[i] = in ? __ldg(row1 + b) : INFINITY;
+      }
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const uint32_t x = __ballot_sync(0xFFFFFFFFu, x0[i] <= p || x1[i] <= p);
+        if (lane == 0 && wb0 + i < nbw) my_bits[wb0 + i] = x;
+      }
     }
     __syncwarp();
     uint32_t* dst = mask_bits + (static_cast<size_t>(h) * NQB + u) * W;
