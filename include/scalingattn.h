@@ -234,6 +234,14 @@ SA_API int sa_get_fwd_variant(void);
 SA_API sa_status sa_fwd_softmax_path_counts(const void* workspace, long long* fixed_host,
                                             long long* exact_host, void* stream);
 
+/* Measurement hook for the roofline of sa_block_significance (bound: the special-function pipe):
+ * runs one launch of a kernel in which every resident warp does nothing but independent
+ * ex2.approx chains (`iters` rounds of 8 per thread) on `stream`, waits for it, and returns its
+ * elapsed milliseconds in *ms_host and the number of exponentials it executed in *n_exp_host (host
+ * pointers). `sink`: device memory, at least 8 * (number of SMs) floats, never written in practice.
+ * Call it in a loop for a sustained-load figure. */
+SA_API sa_status sa_debug_ex2_rate(int iters, float* sink, float* ms_host, double* n_exp_host, void* stream);
+
 /* Debug hook: sa_block_sparse_attn_fwd_ex on a build of the (128,128,128) tcgen05 kernel that also
  * records its walk, so that the union walk of a work item (Alg. 2 re-expressed over the OR of two
  * bit-rows), the numbering of (tile, key block) units and the 64-word window reload can be checked

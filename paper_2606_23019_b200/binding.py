@@ -70,6 +70,8 @@ def load_library() -> C.CDLL:
     lib.sa_block_sparse_attn_fwd_reuse.argtypes = lib.sa_block_sparse_attn_fwd_ex.argtypes
     lib.sa_fwd_softmax_path_counts.restype = ip
     lib.sa_fwd_softmax_path_counts.argtypes = [vp, vp, vp, vp]
+    lib.sa_debug_ex2_rate.restype = ip
+    lib.sa_debug_ex2_rate.argtypes = [ip, vp, vp, vp, vp]
     lib.sa_debug_fwd_walk_log_bytes.restype = sz
     lib.sa_debug_fwd_walk_log_bytes.argtypes = [ip] * 5
     lib.sa_debug_fwd_walk.restype = ip
@@ -307,6 +309,22 @@ def sa_fwd_softmax_path_counts(workspace, stream=None):
     _check(load_library().sa_fwd_softmax_path_counts(_ptr(workspace), C.addressof(a), C.addressof(b),
                                                      _stream(stream)))
     return a.value, b.value
+
+
+def sa_debug_ex2_rate(seconds: float = 0.5, iters: int = 4096, device=None, stream=None):
+    """Measured MUFU.EX2 rate (exponentials per second) under sustained load: launches of the library's
+    ex2-only kernel back to back for about `seconds`; the median rate of the second half is returned."""
+    import time
+    lib = load_library()
+    sink = torch.zeros(8 * 1024, dtype=torch.float32, device=device or "cuda")
+    ms, n = C.c_float(0), C.c_double(0)
+    rates = []
+    t0 = time.time()
+    while time.time() - t0 < seconds or len(rates) < 4:
+        _check(lib.sa_debug_ex2_rate(int(iters), _ptr(sink), C.addressof(ms), C.addressof(n), _stream(stream)))
+        rates.append(n.value / (ms.value * 1e-3))
+    tail = sorted(rates[len(rates) // 2:])
+    return tail[len(tail) // 2]
 
 
 def sa_debug_fwd_walk(q, k, v, mask_bits, Bq: int, Bk: int, scale: float, n_valid=None, stream=None):

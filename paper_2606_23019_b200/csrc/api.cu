@@ -632,6 +632,31 @@ sa_status sa_fwd_softmax_path_counts(const void* workspace, long long* fixed_hos
   return SA_OK;
 }
 
+sa_status sa_debug_ex2_rate(int iters, float* sink, float* ms_host, double* n_exp_host, void* stream) {
+  if (!sink || !ms_host || !n_exp_host || iters <= 0)
+    return fail(SA_ERR_INVALID_ARG, "sa_debug_ex2_rate: bad arguments");
+  sa_status s = check_device();
+  if (s != SA_OK) return s;
+  int n_sm = 0;
+  cudaError_t e = sa::device_sm_count(&n_sm);
+  if (e != cudaSuccess) return cuda_fail(e, "device query");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  cudaEvent_t a = nullptr, b = nullptr;
+  if ((e = cudaEventCreate(&a)) != cudaSuccess || (e = cudaEventCreate(&b)) != cudaSuccess) {
+    if (a) cudaEventDestroy(a);
+    return cuda_fail(e, "cudaEventCreate");
+  }
+  e = cudaEventRecord(a, st);
+  if (e == cudaSuccess) e = sa::launch_ex2_rate(iters, sink, n_sm, st, n_exp_host);
+  if (e == cudaSuccess) e = cudaEventRecord(b, st);
+  if (e == cudaSuccess) e = cudaEventSynchronize(b);
+  if (e == cudaSuccess) e = cudaEventElapsedTime(ms_host, a, b);
+  cudaEventDestroy(a);
+  cudaEventDestroy(b);
+  if (e != cudaSuccess) return cuda_fail(e, "sa_debug_ex2_rate");
+  return SA_OK;
+}
+
 sa_status sa_set_fwd_variant(int variant) {
   if (variant < 0 || variant > 3)
     return fail(SA_ERR_INVALID_ARG, "sa_set_fwd_variant: variant %d not in {0,1,2,3}", variant);

@@ -125,6 +125,7 @@ cudaError_t launch_threshold_update(const float* sig, const float* levels, int n
 cudaError_t launch_fidelity(const float* lse_dense, const float* lse_sparse, const int32_t* rows,
                             int n_rows, int BH, int N, float* fidelity, float* per_row,
                             cudaStream_t st);
+cudaError_t launch_ex2_rate(int iters, float* sink, int n_sm, cudaStream_t st, double* n_exp);
 cudaError_t launch_enumerate(const uint32_t* mask_bits, int H, int NQB, int NKB, int32_t* idx,
                              int32_t* cnt, cudaStream_t st);
 

@@ -35,6 +35,7 @@
 
 #include "common.cuh"
 #include "ptx.cuh"
+#include "trace.cuh"
 
 namespace sa {
 namespace {
@@ -269,12 +270,6 @@ __device__ void producer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, const
 }
 
 // ------------------------------------------------------------------ warp 1: MMA issuer
-#ifdef SA_TRACE
-#define IT_TR(i) { const uint32_t n_ = clock(); itr[i] += n_ - itl; itl = n_; }
-#else
-#define IT_TR(i)
-#endif
-
 // One (query tile, key block) unit whose S has been issued and whose PV is still to come. Every
 // address and descriptor is worked out when the unit is created, BEFORE the issuer blocks on the
 // older unit's P: once P is there, nothing but waits, MMAs and commits lies between it and the
@@ -310,9 +305,7 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
   Pend pd0{}, pd1{};                     // FIFO: pd0 older
   int npend = 0;
   auto bar = [&](const void* b) { return smem_u32(b); };
-#ifdef SA_TRACE
-  uint32_t itr[7] = {0, 0, 0, 0, 0, 0, 0}, itl = clock(), it_units = 0;
-#endif
+  IT_TRACE_DECL
 
   // P arrives in two pieces (p_full + 8 c): the MMAs of a piece are issued as soon as it is in TMEM
   auto issue_pend = [&](const Pend& u) {
@@ -471,9 +464,7 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
         mma_ss_e4<2, 2>(tmem_s, qdesc + (kHalfBytes >> 4), cb.kdesc + (kHalfBytes >> 4), kIdescQK, 1u);
         tc_commit_e(s_full);
         IT_TR(5);
-#ifdef SA_TRACE
-        ++it_units;
-#endif
+        IT_TRACE_UNIT
         if (npend == 0) pd0 = u; else pd1 = u;
         ++npend;
       }
@@ -490,12 +481,7 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     if (npend == 2) pop();
   }
   while (npend > 0) pop();
-#ifdef SA_TRACE
-  if (lane == 0 && blockIdx.x < 2)
-    printf("issuer cta %d units %u: other %u | p_full %u | K %u | V/o_free %u | sched/q %u | S issue %u | PV issue %u (clk per unit)\n",
-           blockIdx.x, it_units, itr[0] / it_units, itr[1] / it_units, itr[2] / it_units, itr[3] / it_units,
-           itr[4] / it_units, itr[5] / it_units, itr[6] / it_units);
-#endif
+  IT_TRACE_REPORT
 }
 
 // P = 2^(c*s - m) of one query row (128 columns in sr), written to TMEM as bf16 in kPChunks pieces
@@ -564,12 +550,7 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
                                          // of s_full[t][.] is consumed in order, none is skipped)
   int sched_n = 0;
   uint32_t n_fixed = 0, n_exact = 0;     // items of this warp by softmax path (p.stats)
-#ifdef SA_TRACE
-  uint32_t tr_acc[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, tr_last = clock(), tr_n = 0, tr_items = 0;
-#define SA_TR(i) { const uint32_t now_ = clock(); tr_acc[i] += now_ - tr_last; tr_last = now_; if (i == 4) ++tr_n; }
-#else
-#define SA_TR(i)
-#endif
+  SA_TRACE_DECL
   // Per item: what the walk needs (the item, its bit-rows, the rows' score bound). next_item() takes
   // the next item from the scheduler ring and waits for its Q tiles; it is called for item n+1
   // BEFORE the epilogue of item n, so that the wait for the Q tiles and the row norms fall into the
@@ -798,9 +779,7 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
       }
       p.lse[grow] = l_run > 0.f ? 0.6931471805599453f * (m_run + lg2(l_run)) : -INFINITY;
       SA_TR(9);
-#ifdef SA_TRACE
-      ++tr_items;
-#endif
+      SA_TRACE_ITEM
     } else {
       const uint4 z = make_uint4(0u, 0u, 0u, 0u);
 #pragma unroll
@@ -812,12 +791,7 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     atomicAdd(p.stats, static_cast<int32_t>(n_fixed));
     atomicAdd(p.stats + 1, static_cast<int32_t>(n_exact));
   }
-#ifdef SA_TRACE
-  if (lane == 0 && blockIdx.x < 2 && quarter == 0)
-    printf("trace cta %d wg %d blocks %u: other %u | wait_s %u | ld %u | max+resc %u | exp+st %u (clk per block); items %u: sched %u | q_full %u | norms %u | o_full %u | epilogue %u (clk per item)\n",
-           blockIdx.x, t, tr_n, tr_acc[0] / tr_n, tr_acc[1] / tr_n, tr_acc[2] / tr_n, tr_acc[3] / tr_n, tr_acc[4] / tr_n,
-           tr_items, tr_acc[5] / tr_items, tr_acc[6] / tr_items, tr_acc[7] / tr_items, tr_acc[8] / tr_items, tr_acc[9] / tr_items);
-#endif
+  SA_TRACE_REPORT
 }
 
 // ------------------------------------------------------------------ kernel
