@@ -37,8 +37,8 @@ UNIT = "TFLOP/s"
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the attention kernel at the bench
 # workload, from the `ncu --set full` capture summarised in profiles/ (None until captured).
-NCU_TRAFFIC_BYTES = {"C4": 3306511304}   # dram__bytes_read.sum + dram__bytes_write.sum, one launch
-NCU_TRAFFIC_SOURCE = {"C4": "profiles/r1f_fwd_tcgen05_c4_full.md"}
+NCU_TRAFFIC_BYTES = {"C4": 3340851008}   # dram__bytes_read.sum + dram__bytes_write.sum, one launch
+NCU_TRAFFIC_SOURCE = {"C4": "profiles/r2_fwd_tcgen05_c4_full.md"}
 
 
 # ------------------------------------------------------------------ pure helpers (CPU-testable)
@@ -375,6 +375,61 @@ def run_west_offline(sa, dev, stream, peaks, log):
     return res
 
 
+def run_dense_library(sa, dev, stream, peaks, log):
+    """Context only (--dense-library): PyTorch's scaled_dot_product_attention (cuDNN backend; library
+    code, not part of this build) on dense bf16 attention at three shapes, next to this kernel at
+    density 1 in the same process -- the stand-in for the paper's dense FlashAttention-3 reference
+    ("<10% overhead at 0% sparsity", 4.8% on long sequences PAPER.md:280, 9.0% at
+    N = 16384 PAPER.md:460)."""
+    import torch
+    import torch.nn.functional as F
+    from torch.nn.attention import SDPBackend, sdpa_kernel
+    rows = []
+    for H, N in ((40, 75648), (12, 65536), (12, 16384)):
+        g = torch.Generator(device=dev).manual_seed(5)
+        q, k, v = [torch.randn((1, H, N, 128), generator=g, device=dev, dtype=torch.float32).to(torch.bfloat16)
+                   for _ in range(3)]
+        scale = float(1.0 / 128 ** 0.5)
+        flops = 4.0 * N * N * 128 * H
+
+        def timed(fn, reps=5):
+            for _ in range(2):
+                fn()
+            torch.cuda.synchronize()
+            ts = []
+            for _ in range(reps):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                fn()
+                b.record(stream)
+                torch.cuda.synchronize()
+                ts.append(a.elapsed_time(b))
+            return statistics.median(ts)
+
+        lib_ms = None
+        try:
+            with sdpa_kernel(SDPBackend.CUDNN_ATTENTION):
+                lib_ms = timed(lambda: F.scaled_dot_product_attention(q, k, v, scale=scale))
+        except RuntimeError as e:                    # backend not available for this shape / build
+            log(f"[bench] dense library (cuDNN) unavailable at H={H} N={N}: {e}")
+        bits = torch.full((H, N // 128, (N // 128 + 31) // 32), -1, dtype=torch.int32, device=dev)
+        out = torch.empty_like(q)
+        lse = torch.empty((1, H, N), dtype=torch.float32, device=dev)
+        ws = torch.empty(max(sa.sa_fwd_workspace_bytes(1, H, N, 128), 256), dtype=torch.uint8, device=dev)
+        ours_ms = timed(lambda: sa.sa_block_sparse_attn_fwd_ex(q, k, v, bits, 128, 128, scale, N, out, lse, ws,
+                                                               stream))
+        row = {"H": H, "N": N, "ours_density1_ms": round(ours_ms, 4),
+               "ours_density1_tflops": round(flops / (ours_ms * 1e-3) / 1e12, 1),
+               "cudnn_sdpa_ms": None if lib_ms is None else round(lib_ms, 4),
+               "cudnn_sdpa_tflops": None if lib_ms is None else round(flops / (lib_ms * 1e-3) / 1e12, 1),
+               "ours_vs_cudnn": None if lib_ms is None else round(ours_ms / lib_ms, 4)}
+        rows.append(row)
+        log(f"[bench] dense library H={H} N={N}: cuDNN SDPA {lib_ms} ms, this kernel at density 1 {ours_ms:.3f} ms")
+        del q, k, v, out, lse, bits
+        torch.cuda.empty_cache()
+    return rows
+
+
 def run_ours(args, rank: int, local_rank: int, world: int) -> int:
     import numpy as np
     import torch
@@ -589,6 +644,10 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> int:
     if rank == 0 and not args.no_west:
         west = run_west_offline(sa, dev, stream, peaks, log)
 
+    dense_lib = None
+    if rank == 0 and args.dense_library:
+        dense_lib = run_dense_library(sa, dev, stream, peaks, log)
+
     # ---- pack-mask kernel group on its own (HBM/ALU-bound; not the dominant kernel)
     pack_ms = None
     if rank == 0:
@@ -730,6 +789,7 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> int:
             "density_sweep": sweep,
             "seqlen_grid": seq_grid,
             "west_offline": west,
+            "dense_library_context": dense_lib,
         }
         print(json.dumps(line), flush=True)
     if dist is not None:
@@ -760,6 +820,9 @@ def main() -> int:
                     help="skip the offline per-sample steps (block significance, threshold-map update, "
                          "fidelity) at Wan2.1-14B 480p shapes")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--dense-library", action="store_true",
+                    help="context only: also time PyTorch SDPA (cuDNN backend, library code) on dense "
+                         "attention next to this kernel at density 1")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     rank = int(os.environ.get("RANK", "0"))
