@@ -7,7 +7,7 @@
  *  - Pointers are DEVICE pointers unless the parameter name ends in _host. The caller owns every
  *    buffer; the library never frees or retains a caller pointer past the stream-ordered end of
  *    the call, and never allocates device memory (scratch comes in as `workspace`; the short
- *    sa_block_sparse_attn_fwd keeps one lazily grown internal workspace per process instead).
+ *    sa_block_sparse_attn_fwd keeps one lazily grown internal workspace per (device, stream) instead).
  *  - `stream` is a cudaStream_t passed as void*. Calls enqueue work on it and return without
  *    synchronising; outputs are valid once the stream reaches the end of the enqueued work.
  *  - Errors are return codes; nothing is launched when validation fails; sa_last_error() holds a
@@ -113,8 +113,8 @@ SA_API sa_status sa_block_significance(const void* q, const void* k, const float
  *   levels : fp32 [n_levels] (device), ascending, in (0, 1], n_levels <= 256 (the candidate set P)
  *   tmap   : fp32 [H][NQB][NKB] (device, in/out); initialise with 1.0 before the first sample
  *   workspace >= sa_threshold_map_update_workspace_bytes(B,H,NQB,NKB) bytes, 256 B aligned.
- * The sort is cub::DeviceSegmentedRadixSort; everything runs on `stream` without synchronising.
- * Deterministic. SA_ERR_UNSUPPORTED if B*H*NQB*NKB >= 2^31 or n_levels > 256. */
+ * The sort is the library's own stable radix sort (13 kernels in all); everything runs on `stream`
+ * without synchronising. Deterministic. SA_ERR_UNSUPPORTED if B*H*NQB*NKB >= 2^31 or n_levels > 256. */
 SA_API size_t sa_threshold_map_update_workspace_bytes(int B, int H, int NQB, int NKB);
 SA_API sa_status sa_threshold_map_update(const float* sig, const float* levels, int n_levels, float* tmap,
                                          int B, int H, int NQB, int NKB, void* workspace,
@@ -144,8 +144,12 @@ SA_API sa_status sa_fidelity_from_lse(const float* lse_dense, const float* lse_s
  * blocks are never loaded and never multiplied. A row with no active key gives out = 0, lse = -inf.
  *   q, k, v, out : bf16 [B][H][N][D] contiguous, 16 B aligned;  lse : fp32 [B][H][N]
  *   scale        : softmax scale (e.g. 1/sqrt(D)); arithmetic is bf16 x bf16 -> fp32.
- * All N tokens are real. Uses an internal workspace (grown with cudaMalloc on first use / when a
- * larger problem arrives, which synchronises; freed at process exit). */
+ * All N tokens are real. Uses an internal workspace per (device, stream): the workspace holds the
+ * scheduler cursor and the work list, which a call rebuilds while an earlier call's kernel may still
+ * be consuming them, so sharing one is only safe in stream order. It is allocated on first use and
+ * when a larger problem arrives, in stream order (cudaMallocAsync / cudaFreeAsync on `stream`, no
+ * synchronisation), and kept until the process exits. Calls from several threads are serialised
+ * across their enqueue (calls sharing a stream then run in the order the lock was taken). */
 SA_API sa_status sa_block_sparse_attn_fwd(const void* q, const void* k, const void* v,
                                    const uint32_t* mask_bits, void* out, float* lse, int B, int H,
                                    int N, int D, int Bq, int Bk, float scale, void* stream);
@@ -215,8 +219,10 @@ SA_API sa_status sa_enumerate_active_blocks(const uint32_t* mask_bits, int H, in
 
 /* Which CUDA kernel the forward pass uses. 0 (default): automatic -- the tcgen05/TMEM/TMA kernel
  * for (128,128,128), the mma.sync kernel for (64,64,64); the tcgen05 kernel takes work items of two
- * adjacent query blocks (shared K/V tiles) unless the problem has fewer than two waves of such pairs,
- * in which case it takes single query blocks. 1: the mma.sync kernel for every supported shape (a
+ * query blocks of one (batch, head) that share their K/V tiles (the schedule pre-pass pairs adjacent
+ * blocks when their popcounts are balanced, otherwise blocks of similar popcount and large bit-row
+ * overlap) unless the problem has fewer than two waves of such pairs, in which case it takes single
+ * query blocks. 1: the mma.sync kernel for every supported shape (a
  * second CUDA implementation kept for cross-checking; not a fallback: it is never chosen implicitly
  * for a shape the fast kernel supports). 2 / 3: the tcgen05 kernel with its large-problem path (pair
  * items, key-norm pre-pass and score bound) / its small-problem path (single-block items, exact running

@@ -6,9 +6,11 @@
 // PAPER.md:484-539). Masked key blocks are never loaded and never multiplied.
 //
 // How (this design is for B200, not the paper's):
-//   * persistent grid, one CTA per SM; a work item is a PAIR of adjacent query blocks (2u, 2u+1)
-//     of one (batch, head). Items are pulled from the popcount-ordered list of the schedule
-//     pre-pass with an atomic cursor, so uneven rows and heads balance out. The producer claims
+//   * persistent grid, one CTA per SM; a work item is a PAIR of query blocks (ua, ub) of one
+//     (batch, head), chosen by the schedule pre-pass (adjacent blocks when their popcounts are
+//     balanced, else partners of similar popcount and large bit-row overlap; schedule.cu). Items
+//     are pulled from the popcount-ordered list of the pre-pass with an atomic cursor, so uneven
+//     rows and heads balance out. The producer claims
 //     one item ahead (2-slot scheduler ring) so the atomic's round trip hides under the current
 //     item's loads; after a long item the claim is taken late instead, so that the tail of the
 //     grid still goes to whichever CTA is free first.
