@@ -221,12 +221,13 @@ SA_API sa_status sa_enumerate_active_blocks(const uint32_t* mask_bits, int H, in
  * for (128,128,128), the mma.sync kernel for (64,64,64); the tcgen05 kernel takes work items of two
  * query blocks of one (batch, head) that share their K/V tiles (the schedule pre-pass pairs adjacent
  * blocks when their popcounts are balanced, otherwise blocks of similar popcount and large bit-row
- * overlap) unless the problem has fewer than two waves of such pairs, in which case it takes single
- * query blocks. 1: the mma.sync kernel for every supported shape (a
+ * overlap); on small problems (fewer than two waves of such pairs, when the rounding to whole items per
+ * SM favours it) it takes single query blocks instead, each SPLIT over the kernel's two tiles (even key
+ * blocks to one, odd to the other, merged in the epilogue). 1: the mma.sync kernel for every supported shape (a
  * second CUDA implementation kept for cross-checking; not a fallback: it is never chosen implicitly
  * for a shape the fast kernel supports). 2 / 3: the tcgen05 kernel with its large-problem path (pair
- * items, key-norm pre-pass and score bound) / its small-problem path (single-block items, exact running
- * max) forced, so that tests can drive either on any size. A DEBUG hook for tests and benchmarks, not
+ * items, key-norm pre-pass and score bound) / its small-problem path (split single-block items, exact
+ * running max) forced, so that tests can drive either on any size. A DEBUG hook for tests and benchmarks, not
  * part of the product surface: process-wide (an atomic read once per call), so it must not be changed
  * while another thread is inside a forward call. The same holds for sa_profile_enable / _collect. */
 SA_API sa_status sa_set_fwd_variant(int variant);

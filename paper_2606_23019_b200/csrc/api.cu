@@ -317,14 +317,23 @@ static sa_status fwd_ex_impl(const void* q, const void* k, const void* v, const 
   // not worth it on problems of a few thousand tiles, which then keep the exact running max
   const bool big = static_cast<long long>(B) * H * p.NQB * p.NKB >= 16384;
   p.kmax2 = (fast && (variant == 2 || (variant == 0 && big))) ? w.kmax2 : nullptr;
-  // The tcgen05 kernel works on PAIRS of query blocks (shared K/V tiles). When there are fewer pairs
-  // than two waves of CTAs (short sequences) single-row items fill the SMs better.
+  // The tcgen05 kernel works on items of two tiles: a PAIR of query blocks that share their K/V tiles,
+  // or ONE query block whose key blocks alternate between the two tiles (a split item, merged in the
+  // epilogue; twice as many items of half the length). With P pairs on n SMs a launch takes about
+  // ceil(P / n) pair items or ceil(2 P / n) split items of half the length per SM: split items are
+  // taken when that rounding favours them and the problem is small (below two waves of pairs); from
+  // there on the dynamic scheduler evens the rounding out and the shared K/V tiles of pairs win
+  // (measured: N = 4096, H = 12 dense 150 -> 131 us with split items, N = 8192 dense 374 us with pairs
+  // against 446 us).
   int n_sm = 0;
   cudaError_t e = sa::device_sm_count(&n_sm);
   if (e != cudaSuccess) return cuda_fail(e, "device query");
   const long long n_pairs = static_cast<long long>(B) * H * ((p.NQB + 1) / 2);
-  const int rows_per_item = (fast && (variant == 2 || (variant == 0 && n_pairs >= 2 * n_sm))) ? 2 : 1;
+  const long long rounds_pairs = 2 * ((n_pairs + n_sm - 1) / n_sm), rounds_split = (2 * n_pairs + n_sm - 1) / n_sm;
+  const bool small = n_pairs < 2LL * n_sm && rounds_split < rounds_pairs;
+  const int rows_per_item = (fast && (variant == 2 || (variant == 0 && !small))) ? 2 : 1;
   p.rows_per_item = rows_per_item;
+  p.split_rows = (fast && rows_per_item == 1) ? 1 : 0;
   p.n_items = B * H * ((p.NQB + rows_per_item - 1) / rows_per_item);
   e = sa::launch_schedule(p, w, rows_per_item, st, &g_last_launches, reuse_schedule);
   if (e != cudaSuccess) return cuda_fail(e, "schedule pre-pass launch");

@@ -66,6 +66,7 @@ struct FwdParams {
   const float* kmax2;         // [B*H] max |k|^2 over the valid keys (tcgen05 kernel only)
   int n_items;                // host-side count: exact for single-row items, an upper bound for pairs
   int rows_per_item;          // query blocks per work item: 2 (a pair shares its K/V tiles) or 1
+  int split_rows;             // single-row items are split items (tcgen05 kernel): see Item::split
   int32_t* stats;             // [2] (warp, item) counts by softmax path: fixed reference point / exact
                               // running max (zeroed by the pre-pass; tcgen05 kernel only)
   int32_t* walk_log;          // sa_debug_fwd_walk only (else null): see WalkLog in fwd_tcgen05.cu

@@ -83,6 +83,7 @@ struct __align__(8) Ctl {
   uint64_t kv_full[kSlots], kv_empty[kSlots];
   uint64_t s_full[2][2], p_full[2][2][4], pv_done[2][2];   // [tile][tile-local unit & 1]
   uint64_t o_full[2], o_free[2];
+  uint64_t xchg_full, xchg_empty;     // split items: warpgroup 1 has published its half / warpgroup 0 has read it
   uint64_t sched_full[kSched], sched_empty[kSched];
   int2 sched_item[kSched];            // item record (x = -1: no more work)
   uint32_t tmem_base;
@@ -114,6 +115,10 @@ struct Item {
   int bh, h, ua, ub;
   bool has1;
   int row0;            // first token row of the (b,h) slab in the [B*H*N][D] view
+  // ub == ua: a SPLIT item -- ONE query block whose key blocks are dealt to the two tiles in turn (even
+  // key blocks -> tile 0, odd -> tile 1), the halves merged in the epilogue. (Derived on demand: the
+  // softmax loop has no register to spare for another live flag.)
+  __device__ __forceinline__ bool split() const { return ub == ua; }
 };
 // item record: x = b*H + h (-1: no more work), y = ua | ub << 16 (ub = 0xFFFF: no second row)
 __device__ __forceinline__ Item decode_item(const FwdParams& p, int2 rec) {
@@ -164,8 +169,15 @@ struct RowWalk {
     const int w0 = base + lane, w1 = base + 32 + lane;
     a0 = w0 < p.W ? row_word(p, it.h, it.ua, w0, true) : 0u;
     a1 = w1 < p.W ? row_word(p, it.h, it.ua, w1, true) : 0u;
-    b0 = w0 < p.W ? row_word(p, it.h, it.ub, w0, it.has1) : 0u;
-    b1 = w1 < p.W ? row_word(p, it.h, it.ub, w1, it.has1) : 0u;
+    if (it.split()) {                    // one row, its key blocks alternating between the tiles
+      b0 = a0 & 0xAAAAAAAAu;
+      b1 = a1 & 0xAAAAAAAAu;
+      a0 &= 0x55555555u;
+      a1 &= 0x55555555u;
+    } else {
+      b0 = w0 < p.W ? row_word(p, it.h, it.ub, w0, it.has1) : 0u;
+      b1 = w1 < p.W ? row_word(p, it.h, it.ub, w1, it.has1) : 0u;
+    }
   }
   // number of set bits of each row within the loaded 64 words
   __device__ __forceinline__ void counts(uint32_t& n0, uint32_t& n1) const {
@@ -236,8 +248,9 @@ __device__ void producer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, const
 
     mbar_wait(smem_u32(&ctl->q_empty), q_phase ^ 1u, 2);
     const uint32_t qf = smem_u32(&ctl->q_full);
-    mbar_expect_tx_e(qf, it.has1 ? 2 * kTileBytes : kTileBytes);
-    for (int t = 0; t < (it.has1 ? 2 : 1); ++t) {
+    const int q_tiles = (it.has1 && !it.split()) ? 2 : 1;      // a split item has one query tile
+    mbar_expect_tx_e(qf, q_tiles * kTileBytes);
+    for (int t = 0; t < q_tiles; ++t) {
       const uint32_t dst = smem_base + kOffQ + t * kTileBytes;
       const int y = it.row0 + (t == 0 ? it.ua : it.ub) * kBlk;
       tma_load_2d_e(dst, tm_q, 0, y, qf);
@@ -439,7 +452,7 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
         u.v_empty = last_of_blk ? cb.v_empty : 0u;
         u.o_full = (--rem[t] == 0u) ? bar(&ctl->o_full[t]) : 0u;
         const uint32_t tmem_s = tmem + buf * 128;
-        const uint64_t qdesc = make_desc(kDescKMajor, smem_base + kOffQ + t * kTileBytes);
+        const uint64_t qdesc = make_desc(kDescKMajor, smem_base + kOffQ + (it.split() ? 0 : t) * kTileBytes);
         const uint32_t s_full = bar(&ctl->s_full[t][sel]);
         if constexpr (kLog) {          // debug build of the kernel (sa_debug_fwd_walk): the issue order
           if (lane == 0) WalkLog(p).is_seq(it.bh * p.NQB + it.ua)[n_logged] = (t << 15) | cb.j;
@@ -552,6 +565,7 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
                                          // of s_full[t][.] is consumed in order, none is skipped)
   int sched_n = 0;
   uint32_t n_fixed = 0, n_exact = 0;     // items of this warp by softmax path (p.stats)
+  uint32_t n_split = 0;                  // split items so far (parity of the xchg barriers)
   SA_TRACE_DECL
   // Per item: what the walk needs (the item, its bit-rows, the rows' score bound). next_item() takes
   // the next item from the scheduler ring and waits for its Q tiles; it is called for item n+1
@@ -588,7 +602,7 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     qf_phase ^= 1u;
     bound = 0.f;
     if (exists) {
-      const uint32_t qrow = smem_base + kOffQ + t * kTileBytes + row * 128;
+      const uint32_t qrow = smem_base + kOffQ + (it.split() ? 0 : t) * kTileBytes + row * 128;
       float qn2 = 0.f;
 #pragma unroll
       for (int ch = 0; ch < 16; ++ch) {
@@ -740,10 +754,79 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
       }
     }
     const bool wrote = exists;
+    const bool split = it.split();
     const size_t grow = static_cast<size_t>(it.row0) + static_cast<size_t>(t == 0 ? it.ua : it.ub) * kBlk + row;
     uint4* orow = reinterpret_cast<uint4*>(p.out + grow * kD);
     have_item = next_item();             // (overwrites it, exists, rw, bound)
     if (!wrote) continue;
+    if (split) {
+      // ---- a split item: the two warpgroups hold the two halves (even / odd key blocks) of ONE query
+      // block, each with its own running maximum, row sum and O tile. Warpgroup 1 publishes (m, l) of
+      // its half -- in the first 8 bytes of the output row, which warpgroup 0 overwrites afterwards --
+      // and leaves its O tile in TMEM; warpgroup 0 (same TMEM lanes) reads both tiles, 32 columns at a
+      // time (no more live registers than the plain epilogue: the per-block loop has none to spare), and
+      // writes  out = (O0 2^(m0-M) + O1 2^(m1-M)) / (l0 2^(m0-M) + l1 2^(m1-M)),  lse = ln2 (M + log2(.)),
+      // M = max(m0, m1): the same softmax, summed in a fixed order (deterministic).
+      float2* xchg = reinterpret_cast<float2*>(orow);
+      if (started) {
+        mbar_wait(smem_u32(&ctl->o_full[t]), o_phase, 22);     // this half's O tile is complete
+        o_phase ^= 1u;
+      }
+      // (hand-off through an mbarrier pair with back-pressure: a half without units publishes at once,
+      // and must not get two items ahead of the reader)
+      if (t == 1) {
+        mbar_wait(smem_u32(&ctl->xchg_empty), (n_split & 1u) ^ 1u, 26);
+        __stcg(xchg, make_float2(started ? m_run : -INFINITY, started ? l_run : -1.f));   // l < 0: no units
+        __threadfence_block();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&ctl->xchg_full));
+        ++n_split;
+        continue;                          // O1 is released by warpgroup 0 once it has read it
+      }
+      mbar_wait(smem_u32(&ctl->xchg_full), n_split & 1u, 27);
+      ++n_split;
+      tc_fence_after();
+      float2 ml1 = __ldcg(xchg);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(smem_u32(&ctl->xchg_empty));
+      const bool other = ml1.y >= 0.f;     // tile 1 had units in this item: its O tile is valid
+      ml1.y = fmaxf(ml1.y, 0.f);
+      const float m0 = started ? m_run : -INFINITY, l0 = started ? l_run : 0.f;
+      const float M = fmaxf(m0, ml1.x);
+      const float a0 = m0 > -INFINITY ? ex2(m0 - M) : 0.f, a1 = ml1.x > -INFINITY ? ex2(ml1.x - M) : 0.f;
+      const float L = l0 * a0 + ml1.y * a1;
+      const float inv = L > 0.f ? 1.f / L : 0.f;
+      const float s0 = started ? a0 * inv : 0.f, s1 = other ? a1 * inv : 0.f;
+#pragma unroll 1
+      for (int cc = 0; cc < 4; ++cc) {
+        uint32_t o0[32], o1[32];
+        tmem_ld32(tm_o + cc * 32, o0);                 // (an unused tile's columns hold old finite data or
+        tmem_ld32(tm_o + 128 + cc * 32, o1);           //  anything at all: its weight below is exactly 0)
+        tc_wait_ld();
+#pragma unroll
+        for (int ch = 0; ch < 4; ++ch) {
+          uint32_t v[4];
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            const int i = 8 * ch + 2 * k;
+            const float x0 = s0 != 0.f ? __uint_as_float(o0[i]) * s0 : 0.f;
+            const float x1 = s0 != 0.f ? __uint_as_float(o0[i + 1]) * s0 : 0.f;
+            const float y0 = s1 != 0.f ? fmaf(__uint_as_float(o1[i]), s1, x0) : x0;
+            const float y1 = s1 != 0.f ? fmaf(__uint_as_float(o1[i + 1]), s1, x1) : x1;
+            v[k] = pack_bf16x2(y0, y1);
+          }
+          orow[cc * 4 + ch] = make_uint4(v[0], v[1], v[2], v[3]);
+        }
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) {
+        if (started) mbar_arrive(smem_u32(&ctl->o_free[0]));
+        if (other) mbar_arrive(smem_u32(&ctl->o_free[1]));
+      }
+      p.lse[grow] = L > 0.f ? 0.6931471805599453f * (M + lg2(L)) : -INFINITY;
+      continue;
+    }
     if (started) {
       SA_TR(0);
       mbar_wait(smem_u32(&ctl->o_full[t]), o_phase, 22);
@@ -827,6 +910,10 @@ fwd_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
       }
       mbar_init(smem_u32(&ctl->o_full[t]), 1);
       mbar_init(smem_u32(&ctl->o_free[t]), 4);
+      if (t == 0) {
+        mbar_init(smem_u32(&ctl->xchg_full), 4);     // one arrival per warp of warpgroup 1
+        mbar_init(smem_u32(&ctl->xchg_empty), 4);    // one arrival per warp of warpgroup 0
+      }
     }
     for (int s = 0; s < kSched; ++s) {
       mbar_init(smem_u32(&ctl->sched_full[s]), 1);

@@ -111,7 +111,7 @@ __device__ __forceinline__ int pow2_at_least(int n) {
 // Dynamic shared memory: keys[n2] (uint32), then pop[NQB], ia[slots], ib[slots] (uint16).
 __global__ void __launch_bounds__(kSortThreads)
 schedule_items_kernel(const uint32_t* __restrict__ mask_bits, int H, int NQB, int NKB, int W,
-                      int pair_rows, int n2, int32_t* __restrict__ head_cost,
+                      int pair_rows, int split_rows, int n2, int32_t* __restrict__ head_cost,
                       int32_t* __restrict__ head_count, int2* __restrict__ local_items,
                       float* __restrict__ kmax2) {
   extern __shared__ uint32_t s_dyn[];
@@ -254,8 +254,11 @@ schedule_items_kernel(const uint32_t* __restrict__ mask_bits, int H, int NQB, in
   for (int pos = threadIdx.x; pos < count; pos += blockDim.x) {
     const uint32_t key = s_keys[pos];
     const int s = static_cast<int>(kIdxMask - (key & kIdxMask));
+    // single-row items of the tcgen05 kernel are SPLIT items (ub = ua): the row's key blocks go to
+    // the kernel's two tiles in turn, so both softmax warpgroups work on the one row
+    const int ub = (!pair_rows && split_rows) ? s_a[s] : s_b[s];
     local_items[static_cast<size_t>(bh) * NQB + pos] =
-        make_int2(static_cast<int>(key >> kIdxBits) - 1, s_a[s] | (static_cast<int>(s_b[s]) << 16));
+        make_int2(static_cast<int>(key >> kIdxBits) - 1, s_a[s] | (ub << 16));
   }
   if (threadIdx.x == 0) {
     head_cost[bh] = s_total;
@@ -392,7 +395,8 @@ cudaError_t launch_schedule(const FwdParams& p, const FwdWorkspace& w, int rpi, 
       if (e != cudaSuccess) return e;
     }
     schedule_items_kernel<<<BH, kSortThreads, smem, st>>>(p.mask_bits, p.H, p.NQB, p.NKB, p.W, rpi == 2 ? 1 : 0,
-                                                         n2, w.head_cost, w.head_count, w.local_items, w.kmax2);
+                                                         p.split_rows, n2, w.head_cost, w.head_count,
+                                                         w.local_items, w.kmax2);
     *n_launch += 1;
   }
   if (!reuse || norms) {
