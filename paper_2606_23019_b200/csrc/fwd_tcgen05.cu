@@ -652,7 +652,7 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
       for (;;) {
         const int j = w * 32 + bit;
         if constexpr (kLog) {
-          if (quarter == 0 && lane == 0)
+          if (quarter == 0 && lane == 0 && !(t == 1 && it.split()))   // a split item's row: tile 0 logs
             WalkLog(p).wg_seq(static_cast<size_t>(it.bh) * p.NQB + (t == 0 ? it.ua : it.ub))[n_logged] =
                 static_cast<int32_t>(((my - wg_item0) << 16) | static_cast<uint32_t>(j));
           ++n_logged;
@@ -746,7 +746,7 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
 
     // ---- epilogue: O / l -> bf16, lse = ln2 * (m + log2 l); empty row -> 0 / -inf
     if constexpr (kLog) {
-      if (exists && quarter == 0 && lane == 0) {
+      if (exists && quarter == 0 && lane == 0 && !(t == 1 && it.split())) {
         const size_t lrow = static_cast<size_t>(it.bh) * p.NQB + (t == 0 ? it.ua : it.ub);
         const int partner = t == 0 ? (it.has1 ? it.ub : -1) : it.ua;
         WalkLog(p).wg_cnt()[lrow] = n_logged;

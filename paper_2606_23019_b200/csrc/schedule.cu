@@ -219,12 +219,14 @@ schedule_items_kernel(const uint32_t* __restrict__ mask_bits, int H, int NQB, in
           if (s2 > best) { p0 = 3; p1 = 1; p2 = 2; }
         }
         if (lane == 0) {
+          // a row left without a partner becomes a split item (ub = ua): its key blocks alternate
+          // between the kernel's two tiles, so that both softmax warpgroups work on it
           const int s = n_adj + 2 * g;
           s_a[s] = static_cast<uint16_t>(r[0]);
-          s_b[s] = r[p0] >= 0 ? static_cast<uint16_t>(r[p0]) : 0xFFFFu;
+          s_b[s] = static_cast<uint16_t>(r[p0] >= 0 ? r[p0] : r[0]);
           if (r[p1] >= 0) {
             s_a[s + 1] = static_cast<uint16_t>(r[p1]);
-            s_b[s + 1] = r[p2] >= 0 ? static_cast<uint16_t>(r[p2]) : 0xFFFFu;
+            s_b[s + 1] = static_cast<uint16_t>(r[p2] >= 0 ? r[p2] : r[p1]);
           }
         }
       }
@@ -243,7 +245,7 @@ schedule_items_kernel(const uint32_t* __restrict__ mask_bits, int H, int NQB, in
   for (int s = threadIdx.x; s < min(used, slots); s += blockDim.x) {
     const int a = s_a[s], b = s_b[s];
     if (a == 0xFFFF) continue;
-    const int cost = s_pop[a] + (b != 0xFFFF ? s_pop[b] : 0);
+    const int cost = s_pop[a] + ((b != 0xFFFF && b != a) ? s_pop[b] : 0);
     s_keys[s] = (static_cast<uint32_t>(cost + 1) << kIdxBits) | (kIdxMask - s);
     ++mine;
   }

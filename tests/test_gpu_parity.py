@@ -131,15 +131,22 @@ def test_tcgen05_union_walk_matches_cpu_enumeration(sa, nkb):
             assert not seen[h, u]
             seen[h, u] = True
             a, b = (u, partner) if t == 0 else (partner, u)
-            assert a >= 0 and (b < 0 or (b != a and 0 <= b < nqb))
-            if b >= 0:                          # the partner names this row as its partner, other tile
+            assert a >= 0 and (b < 0 or 0 <= b < nqb)
+            split = b == a                      # a row without a partner: its own key blocks alternate
+            if b >= 0 and not split:            # the partner names this row as its partner, other tile
                 rp = h * nqb + partner
                 assert (int(wg_info[rp]) >> 1) - 1 == u and (int(wg_info[rp]) & 1) == 1 - t
                 n_pairs += 1
             # CPU enumeration of the item's walk from the boolean mask: key blocks ascending, tile 0
-            # before tile 1 on a key block both rows have; units numbered in that order
-            ja = np.nonzero(dense[h, a])[0]
-            jb = np.nonzero(dense[h, b])[0] if b >= 0 else np.zeros(0, dtype=np.int64)
+            # before tile 1 on a key block both rows have; units numbered in that order. A split item
+            # deals the row's even key blocks to tile 0 and the odd ones to tile 1 (tile 0 logs).
+            if split:
+                assert t == 0
+                jj = np.nonzero(dense[h, a])[0]
+                ja, jb = jj[jj % 2 == 0], jj[jj % 2 == 1]
+            else:
+                ja = np.nonzero(dense[h, a])[0]
+                jb = np.nonzero(dense[h, b])[0] if b >= 0 else np.zeros(0, dtype=np.int64)
             js = np.concatenate([ja, jb])
             ts = np.concatenate([np.zeros(len(ja), dtype=np.int64), np.ones(len(jb), dtype=np.int64)])
             order = np.lexsort((ts, js))
