@@ -110,7 +110,7 @@ cudaError_t launch_fwd_tcgen05(const FwdParams& p, void* ws_extra, cudaStream_t 
 cudaError_t launch_pack_mask(const float* scores, const float* density, uint32_t* mask_bits, int H,
                              int NQB, int NKB, int force_diag, void* ws, cudaStream_t st);
 size_t pack_mask_workspace_bytes(int H, int NQB, int NKB);
-constexpr int kPackMaskLaunches = 6;   // kernels launch_pack_mask enqueues (plus one memset)
+constexpr int kPackMaskLaunches = 5;   // kernels launch_pack_mask enqueues (plus one memset)
 cudaError_t launch_mask_from_threshold(const float* tmap, const float* p_star, uint32_t* mask_bits,
                                        int H, int nbq, int nbk, int NQB, int NKB, int force_diag,
                                        cudaStream_t st);
