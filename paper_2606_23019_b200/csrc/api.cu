@@ -136,9 +136,20 @@ size_t sa_pack_mask_workspace_bytes(int H, int NQB, int NKB) {
   return sa::pack_mask_workspace_bytes(H, NQB, NKB);
 }
 
+// The workspace holds room for the parts of the last round's rows (sa::fwd_tail_plan), which depends
+// on the SM count of the current device (148 when no device can be queried: sizing only).
+static sa::TailPlan sized_tail_plan(int B, int H, int NQB) {
+  int n_sm = 0;
+  if (sa::device_sm_count(&n_sm) != cudaSuccess || n_sm <= 0) {
+    (void)cudaGetLastError();
+    n_sm = 148;
+  }
+  return sa::fwd_tail_plan(B, H, NQB, NQB < 0xFFFF ? NQB : 0xFFFF, n_sm);   // (the fast path has Bq == Bk)
+}
+
 size_t sa_fwd_workspace_bytes(int B, int H, int N, int Bq) {
   if (B <= 0 || H <= 0 || N <= 0 || Bq <= 0 || N % Bq != 0) return 0;
-  return sa::fwd_workspace_bytes(B, H, N / Bq);
+  return sa::fwd_workspace_bytes(B, H, N / Bq, (N / Bq + 31) / 32, sized_tail_plan(B, H, N / Bq));   // (Bq == Bk where parts exist)
 }
 
 static size_t al256(size_t x) { return (x + 255) / 256 * 256; }
@@ -286,7 +297,8 @@ static sa_status fwd_ex_impl(const void* q, const void* k, const void* v, const 
   if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out) || !mask_ok ||
       !aligned16(lse) || !aligned16(workspace))
     return fail(SA_ERR_INVALID_ARG, "sa_block_sparse_attn_fwd: pointers must be 16-byte aligned");
-  const size_t need = sa::fwd_workspace_bytes(B, H, N / Bq);
+  const sa::TailPlan sized_plan = sized_tail_plan(B, H, N / Bq);
+  const size_t need = sa::fwd_workspace_bytes(B, H, N / Bq, (N / Bq + 31) / 32, sized_plan);
   if (!workspace || workspace_bytes < need)
     return fail(SA_ERR_WORKSPACE, "sa_block_sparse_attn_fwd: workspace %zu B < %zu B",
                 workspace_bytes, need);
@@ -305,7 +317,7 @@ static sa_status fwd_ex_impl(const void* q, const void* k, const void* v, const 
   p.NQB = N / Bq; p.NKB = N / Bk; p.W = (p.NKB + 31) / 32;
   p.scale = scale;
   p.scale_log2 = scale * 1.4426950408889634f;
-  const sa::FwdWorkspace w = sa::carve_fwd_workspace(workspace, B, H, p.NQB);
+  const sa::FwdWorkspace w = sa::carve_fwd_workspace(workspace, B, H, p.NQB, (p.NQB + 31) / 32, sized_plan);
   p.items = w.items;
   p.n_items_dev = w.n_items;
   p.counter = w.cursor;
@@ -334,8 +346,14 @@ static sa_status fwd_ex_impl(const void* q, const void* k, const void* v, const 
   const int rows_per_item = (fast && (variant == 2 || (variant == 0 && !small))) ? 2 : 1;
   p.rows_per_item = rows_per_item;
   p.split_rows = (fast && rows_per_item == 1) ? 1 : 0;
-  p.n_items = B * H * ((p.NQB + rows_per_item - 1) / rows_per_item);
-  e = sa::launch_schedule(p, w, rows_per_item, st, &g_last_launches, reuse_schedule);
+  // the partly filled last round of pair items is issued in parts over key ranges (schedule.cu)
+  const sa::TailPlan plan = (fast && variant == 0 && rows_per_item == 2 && p.NKB <= 0xFFFF)
+                                ? sa::fwd_tail_plan(B, H, p.NQB, p.NKB, n_sm) : sa::TailPlan{};
+  p.part_mask = w.part_mask;
+  p.part_out = w.part_out;
+  p.part_lse = w.part_lse;
+  p.n_items = B * H * ((p.NQB + rows_per_item - 1) / rows_per_item) + plan.rem * (plan.parts - (plan.parts ? 1 : 0));
+  e = sa::launch_schedule(p, w, rows_per_item, plan, st, &g_last_launches, reuse_schedule);
   if (e != cudaSuccess) return cuda_fail(e, "schedule pre-pass launch");
   cudaEvent_t ev_stop = nullptr;
   {
@@ -351,6 +369,8 @@ static sa_status fwd_ex_impl(const void* q, const void* k, const void* v, const 
     const char* txt = nullptr;
     e = sa::launch_fwd_tcgen05(p, nullptr, st, &g_last_launches, &txt);
     if (e != cudaSuccess) return cuda_fail(e, txt ? txt : "tcgen05 forward launch");
+    e = sa::launch_combine_parts(p, w, plan, st, &g_last_launches);
+    if (e != cudaSuccess) return cuda_fail(e, "combine launch");
   } else {
     e = sa::launch_fwd_mma_sync(p, st, &g_last_launches);
     if (e != cudaSuccess) return cuda_fail(e, "mma.sync forward launch");

@@ -59,8 +59,12 @@ struct FwdParams {
   float scale;
   float scale_log2;   // scale * log2(e)
   // schedule (workspace)
-  const int2* items;          // work items in issue order: x = b*H + h, y = ua | ub << 16 (query blocks
-                              // of the item; ub = 0xFFFF: single-row item)
+  const int4* items;          // work items in issue order: x = b*H + h, y = ua | ub << 16 (query blocks
+                              // of the item; ub = 0xFFFF: single-row item), z = scratch slot of a
+                              // part (-1: whole rows)
+  const uint32_t* part_mask;  // parts of rows: [slot][tile][W] the bit-rows restricted to the part's key range
+  __nv_bfloat16* part_out;    // parts of rows (tcgen05 kernel): [slot][tile][128][D] normalised O
+  float* part_lse;            //                                  [slot][tile][128] lse of the part
   const int32_t* n_items_dev; // number of work items, written by the pre-pass (pair items: mask-dependent)
   int32_t* counter;           // dynamic scheduler cursor (zeroed by the pre-pass)
   const float* kmax2;         // [B*H] max |k|^2 over the valid keys (tcgen05 kernel only)
@@ -79,20 +83,35 @@ struct FwdParams {
 //   [16 .. 16+BH)        per-(b,h) total cost (active tiles)
 //   [.. + BH)            per-(b,h) number of items
 //   [.. + BH)            fp32: per (b,h) max over the valid keys of |k|^2
-//   int2 [BH*NQB]        per-(b,h) items, cost descending: {cost, ua | ub << 16}
-//   int2 [BH*NQB]        all items in issue order: {b*H + h, ua | ub << 16}
+//   [.. + BH)            per-(b,h) number of items at the tail of the issue order
+//   int4 [BH*NQB]        per-(b,h) items, cost descending: {cost, ua | ub << 16, part slot or -1, 0}
+//   int4 [BH*NQB]        all items in issue order: {b*H + h, ua | ub << 16, part slot or -1, 0}
+//   int4 [rem]           rows issued in parts: {b*H + h (-1: not split after all), ua | ub << 16, parts, first slot}
+//   uint32               [rem * parts][2][W] the parts' bit-rows (the rows' bits inside the part's key range)
+//   bf16 / fp32          part results: [rem * parts][2][128][128] O and [rem * parts][2][128] lse
+// TailPlan: the last, partly filled round of pair items over the SMs is cut into key ranges: `rem`
+// pairs (spread over the (b,h) groups, each group's lightest) are issued in `parts` parts each.
+struct TailPlan {
+  int rem = 0, parts = 0;
+};
+TailPlan fwd_tail_plan(int B, int H, int NQB, int NKB, int n_sm);
 struct FwdWorkspace {
   int32_t* cursor;
   int32_t* n_items;
   int32_t* stats;
   int32_t* head_cost;
   int32_t* head_count;
+  int32_t* head_tail;         // [B*H] how many of the group's items go to the tail of the issue order
   float* kmax2;               // [B*H] max over valid keys of |k|^2
-  int2* local_items;
-  int2* items;
+  int4* local_items;
+  int4* items;
+  int4* tasks;                // [plan.rem] rows issued in parts
+  uint32_t* part_mask;
+  __nv_bfloat16* part_out;
+  float* part_lse;
 };
-size_t fwd_workspace_bytes(int B, int H, int NQB);
-FwdWorkspace carve_fwd_workspace(void* ws, int B, int H, int NQB);
+size_t fwd_workspace_bytes(int B, int H, int NQB, int W, TailPlan plan);
+FwdWorkspace carve_fwd_workspace(void* ws, int B, int H, int NQB, int W, TailPlan plan);
 
 // per-device state (device.cu): SM count of the current device; dynamic shared-memory opt-in of a
 // kernel, set once per (device, kernel)
@@ -101,9 +120,35 @@ enum SmemKernel { kSmemFwdTcgen05 = 0, kSmemFwdTcgen05Log, kSmemSigTcgen05, kSme
 cudaError_t device_sm_count(int* n_sm);
 cudaError_t ensure_dynamic_smem(SmemKernel id, const void* func, int bytes);
 
+// Programmatic dependent launch: the kernel may be scheduled while its predecessor on the stream is
+// still running (its launch latency and prologue overlap the predecessor's tail); it must execute
+// griddep_wait() before it reads anything the predecessor (or anything before that) wrote.
+__device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
+                              Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+#ifdef SA_NO_PDL
+  cfg.numAttrs = 0;
+#else
+  cfg.numAttrs = 1;
+#endif
+  return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 // launchers (each returns the cudaError_t of its launches; *n_launch += kernels enqueued)
 cudaError_t launch_schedule(const FwdParams& p, const FwdWorkspace& w, int rows_per_item,
-                            cudaStream_t st, int* n_launch, bool reuse = false);
+                            TailPlan plan, cudaStream_t st, int* n_launch, bool reuse = false);
+cudaError_t launch_combine_parts(const FwdParams& p, const FwdWorkspace& w, TailPlan plan,
+                                 cudaStream_t st, int* n_launch);
 cudaError_t launch_fwd_mma_sync(const FwdParams& p, cudaStream_t st, int* n_launch);
 cudaError_t launch_fwd_tcgen05(const FwdParams& p, void* ws_extra, cudaStream_t st, int* n_launch,
                                const char** err_text);

@@ -88,7 +88,7 @@ __global__ void __launch_bounds__(BLK * 2, 1) fwd_mma_sync_kernel(const FwdParam
   const uint32_t sK0 = sQ + TILE_BYTES;            // K[2]
   const uint32_t sV0 = sK0 + 2 * TILE_BYTES;       // V[2]
 
-  const int2 item = p.items[blockIdx.x];       // single-row items: x = b*H + h, y = query block | 0xFFFF << 16
+  const int4 item = p.items[blockIdx.x];       // single-row items: x = b*H + h, y = query block | 0xFFFF << 16
   const int bh = item.x, u = item.y & 0xFFFF;
   const int h = bh % p.H;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;

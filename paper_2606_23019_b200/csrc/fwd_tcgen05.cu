@@ -85,7 +85,7 @@ struct __align__(8) Ctl {
   uint64_t o_full[2], o_free[2];
   uint64_t xchg_full, xchg_empty;     // split items: warpgroup 1 has published its half / warpgroup 0 has read it
   uint64_t sched_full[kSched], sched_empty[kSched];
-  int2 sched_item[kSched];            // item record (x = -1: no more work)
+  int4 sched_item[kSched];            // item record (x = -1: no more work)
   uint32_t tmem_base;
 };
 constexpr uint32_t kSmemBytes = kOffCtl + sizeof(Ctl) + 1024;   // + alignment slack
@@ -115,13 +115,16 @@ struct Item {
   int bh, h, ua, ub;
   bool has1;
   int row0;            // first token row of the (b,h) slab in the [B*H*N][D] view
+  int part;            // >= 0: a PART of its rows (a key range of them): the bit-rows restricted to the range
+                       // are rows 2 part, 2 part + 1 of p.part_mask, the results go to scratch slot `part`
   // ub == ua: a SPLIT item -- ONE query block whose key blocks are dealt to the two tiles in turn (even
   // key blocks -> tile 0, odd -> tile 1), the halves merged in the epilogue. (Derived on demand: the
   // softmax loop has no register to spare for another live flag.)
   __device__ __forceinline__ bool split() const { return ub == ua; }
 };
-// item record: x = b*H + h (-1: no more work), y = ua | ub << 16 (ub = 0xFFFF: no second row)
-__device__ __forceinline__ Item decode_item(const FwdParams& p, int2 rec) {
+// item record: x = b*H + h (-1: no more work), y = ua | ub << 16 (ub = 0xFFFF: no second row),
+// z = scratch slot of a part (-1: the item covers its rows' whole bit-rows and writes out / lse itself)
+__device__ __forceinline__ Item decode_item(const FwdParams& p, int4 rec) {
   Item it;
   it.bh = rec.x;
   it.h = it.bh % p.H;
@@ -129,6 +132,7 @@ __device__ __forceinline__ Item decode_item(const FwdParams& p, int2 rec) {
   it.ub = (rec.y >> 16) & 0xFFFF;
   it.has1 = it.ub != 0xFFFF;
   it.row0 = it.bh * p.N;
+  it.part = rec.z;
   return it;
 }
 
@@ -150,10 +154,14 @@ struct WalkLog {
   __device__ int32_t* is_seq(size_t row) const { return base + 3 * rows + rows * nkb + row * 2 * nkb; }
 };
 
-// word w of the bit-row of query block u (0 beyond the grid), stray high bits cleared
-__device__ __forceinline__ uint32_t row_word(const FwdParams& p, int h, int u, int w, bool exists) {
+// word w of the bit-row of query block u (0 beyond the grid), stray high bits cleared; for a part,
+// of the row's copy that holds the part's key range only (written by the schedule pre-pass)
+__device__ __forceinline__ uint32_t row_word(const FwdParams& p, int h, int u, int w, bool exists,
+                                             int part, int tile) {
   if (!exists) return 0u;
-  uint32_t x = __ldg(p.mask_bits + (static_cast<size_t>(h) * p.NQB + u) * p.W + w);
+  const uint32_t* row = part < 0 ? p.mask_bits + (static_cast<size_t>(h) * p.NQB + u) * p.W
+                                 : p.part_mask + static_cast<size_t>(2 * part + tile) * p.W;
+  uint32_t x = __ldg(row + w);
   if (w == p.W - 1 && (p.NKB & 31)) x &= (1u << (p.NKB & 31)) - 1u;
   return x;
 }
@@ -167,16 +175,16 @@ struct RowWalk {
   uint32_t a0 = 0, a1 = 0, b0 = 0, b1 = 0;
   __device__ __forceinline__ void load(const FwdParams& p, const Item& it, int base, int lane) {
     const int w0 = base + lane, w1 = base + 32 + lane;
-    a0 = w0 < p.W ? row_word(p, it.h, it.ua, w0, true) : 0u;
-    a1 = w1 < p.W ? row_word(p, it.h, it.ua, w1, true) : 0u;
+    a0 = w0 < p.W ? row_word(p, it.h, it.ua, w0, true, it.part, 0) : 0u;
+    a1 = w1 < p.W ? row_word(p, it.h, it.ua, w1, true, it.part, 0) : 0u;
     if (it.split()) {                    // one row, its key blocks alternating between the tiles
       b0 = a0 & 0xAAAAAAAAu;
       b1 = a1 & 0xAAAAAAAAu;
       a0 &= 0x55555555u;
       a1 &= 0x55555555u;
     } else {
-      b0 = w0 < p.W ? row_word(p, it.h, it.ub, w0, it.has1) : 0u;
-      b1 = w1 < p.W ? row_word(p, it.h, it.ub, w1, it.has1) : 0u;
+      b0 = w0 < p.W ? row_word(p, it.h, it.ub, w0, it.has1, it.part, 1) : 0u;
+      b1 = w1 < p.W ? row_word(p, it.h, it.ub, w1, it.has1, it.part, 1) : 0u;
     }
   }
   // number of set bits of each row within the loaded 64 words
@@ -217,7 +225,7 @@ __device__ void producer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, const
     int idx = 0;
     if (lane == 0) idx = atomicAdd(p.counter, 1);
     idx = __shfl_sync(0xFFFFFFFFu, idx, 0);
-    const int2 it_id = idx < n_items ? __ldg(p.items + idx) : make_int2(-1, 0);
+    const int4 it_id = idx < n_items ? __ldg(p.items + idx) : make_int4(-1, 0, -1, 0);
     const int ss = sched_n % kSched;
     mbar_wait(smem_u32(&ctl->sched_empty[ss]), ((sched_n / kSched) & 1) ^ 1u, 1);
     if (lane == 0) {
@@ -228,9 +236,9 @@ __device__ void producer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, const
     ++sched_n;
     return it_id;
   };
-  int2 next_item = claim_and_publish();
+  int4 next_item = claim_and_publish();
   for (;;) {
-    const int2 item = next_item;
+    const int4 item = next_item;
     if (item.x < 0) break;
     const Item it = decode_item(p, item);
     // ... unless this item is a long one (a held-back item would then wait that long while another
@@ -354,9 +362,11 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     mbar_wait(smem_u32(&ctl->sched_full[ss]), (sched_n / kSched) & 1, 10);
     IT_TR(4);
     // warp-uniform by construction; the reduction tells the compiler so (see uni())
-    int2 item;
+    int4 item;
     item.x = static_cast<int>(uni(static_cast<uint32_t>(ctl->sched_item[ss].x)));
     item.y = static_cast<int>(uni(static_cast<uint32_t>(ctl->sched_item[ss].y)));
+    item.z = static_cast<int>(uni(static_cast<uint32_t>(ctl->sched_item[ss].z)));
+    item.w = 0;
     __syncwarp();
     if (lane == 0) mbar_arrive(smem_u32(&ctl->sched_empty[ss]));
     ++sched_n;
@@ -580,7 +590,7 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     SA_TR(0);
     mbar_wait(smem_u32(&ctl->sched_full[ss]), (sched_n / kSched) & 1, 20);
     SA_TR(5);
-    const int2 item = ctl->sched_item[ss];
+    const int4 item = ctl->sched_item[ss];
     __syncwarp();
     if (lane == 0) mbar_arrive(smem_u32(&ctl->sched_empty[ss]));
     ++sched_n;
@@ -755,8 +765,13 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     }
     const bool wrote = exists;
     const bool split = it.split();
-    const size_t grow = static_cast<size_t>(it.row0) + static_cast<size_t>(t == 0 ? it.ua : it.ub) * kBlk + row;
-    uint4* orow = reinterpret_cast<uint4*>(p.out + grow * kD);
+    // a part of a row (one key range of it) leaves its normalised O and its lse in scratch slot
+    // `part`; combine_parts_kernel (next on the stream) merges the row's parts into out / lse
+    const size_t grow = it.part < 0
+        ? static_cast<size_t>(it.row0) + static_cast<size_t>(t == 0 ? it.ua : it.ub) * kBlk + row
+        : static_cast<size_t>(2 * it.part + (split ? 0 : t)) * kBlk + row;
+    uint4* orow = reinterpret_cast<uint4*>((it.part < 0 ? p.out : p.part_out) + grow * kD);
+    float* lrow = (it.part < 0 ? p.lse : p.part_lse) + grow;
     have_item = next_item();             // (overwrites it, exists, rw, bound)
     if (!wrote) continue;
     if (split) {
@@ -824,10 +839,8 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
         if (started) mbar_arrive(smem_u32(&ctl->o_free[0]));
         if (other) mbar_arrive(smem_u32(&ctl->o_free[1]));
       }
-      p.lse[grow] = L > 0.f ? 0.6931471805599453f * (M + lg2(L)) : -INFINITY;
-      continue;
-    }
-    if (started) {
+      *lrow = L > 0.f ? 0.6931471805599453f * (M + lg2(L)) : -INFINITY;
+    } else if (started) {
       SA_TR(0);
       mbar_wait(smem_u32(&ctl->o_full[t]), o_phase, 22);
       SA_TR(8);
@@ -862,14 +875,14 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
           }
         }
       }
-      p.lse[grow] = l_run > 0.f ? 0.6931471805599453f * (m_run + lg2(l_run)) : -INFINITY;
+      *lrow = l_run > 0.f ? 0.6931471805599453f * (m_run + lg2(l_run)) : -INFINITY;
       SA_TR(9);
       SA_TRACE_ITEM
     } else {
       const uint4 z = make_uint4(0u, 0u, 0u, 0u);
 #pragma unroll
       for (int i = 0; i < 16; ++i) orow[i] = z;
-      p.lse[grow] = -INFINITY;
+      *lrow = -INFINITY;
     }
   }
   if (p.stats != nullptr && lane == 0) {
@@ -929,6 +942,7 @@ fwd_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = ctl->tmem_base;
+  griddep_wait();      // barriers, TMEM and tensor maps were set up under the pre-pass's tail
 
   if (warp < 4) {
     setmaxnreg_dec<88>();
@@ -1002,8 +1016,9 @@ cudaError_t launch_fwd_tcgen05(const FwdParams& p, void*, cudaStream_t st, int* 
     return cudaErrorInvalidValue;
   }
   const int grid = p.n_items < n_sm ? p.n_items : n_sm;   // n_items: upper bound (pairs are mask-dependent)
-  if (log) fwd_tcgen05_kernel<true><<<grid, kThreads, kSmemBytes, st>>>(tq, tk, tv, p);
-  else fwd_tcgen05_kernel<false><<<grid, kThreads, kSmemBytes, st>>>(tq, tk, tv, p);
+  e = log ? launch_pdl(fwd_tcgen05_kernel<true>, dim3(grid), dim3(kThreads), kSmemBytes, st, tq, tk, tv, p)
+          : launch_pdl(fwd_tcgen05_kernel<false>, dim3(grid), dim3(kThreads), kSmemBytes, st, tq, tk, tv, p);
+  if (e != cudaSuccess) return e;
   *n_launch += 1;
   return cudaGetLastError();
 }

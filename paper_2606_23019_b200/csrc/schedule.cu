@@ -15,19 +15,63 @@
 //   * (b,h) groups heaviest first (keeps the concurrently running CTAs on one or two heads, whose
 //     K/V then stay in L2) and, inside a group, items by descending cost (longest-processing-time
 //     first; the tail is the lightest items of the lightest head).
+//   * when the pairs do not fill a whole number of rounds over the SMs and there are few rounds
+//     (fwd_tail_plan), the lightest items of every group -- as many in total as the last round
+//     holds -- are issued in 2 or 4 PARTS each: the same rows over consecutive key ranges that
+//     hold equal shares of the item's key blocks, at the very end of the order, so that the last
+//     round is a half or a quarter as long. A part leaves its normalised O and its lse in a
+//     scratch slot; combine_parts_kernel merges the parts of a row (a fixed order: deterministic).
 // Everything here is integer work on the packed mask only; the resulting order cannot change any
 // output bit (each query block is reduced by one CTA over its key blocks in ascending order).
 #include "common.cuh"
 
 namespace sa {
 
-size_t fwd_workspace_bytes(int B, int H, int NQB) {
-  const size_t BH = static_cast<size_t>(B) * H;
-  const size_t words = 18 + 3 * BH + 4 * BH * static_cast<size_t>(NQB);   // two int2 arrays of BH*NQB records (+ alignment)
-  return ((words * sizeof(int32_t) + 255) / 256) * 256;
+// a part's fixed cost is ~4 key blocks' worth: no shorter parts than this (measured: parts of 16-25
+// key blocks lose 1-2% at density 0.05-0.1)
+constexpr int kMinPartBlocks = 32;
+
+// Pairs that do not fill a whole number of rounds over the SMs: with few rounds the partly filled
+// last one is a large share of the launch (N = 16384, H = 12: 768 pairs = 5 rounds of 148 + 28 pairs,
+// the sixth round as long as the others). Its pairs are issued in 2 or 4 parts (key ranges with the
+// same share of the pair's key blocks), whichever makes ceil(rem * parts / n_sm) / parts, the length of
+// that round in units of a pair, smallest; combine_parts_kernel merges a row's parts afterwards.
+TailPlan fwd_tail_plan(int B, int H, int NQB, int NKB, int n_sm) {
+  TailPlan t;
+  const long long groups = static_cast<long long>(B) * H;
+  const long long n_pairs = groups * ((NQB + 1) / 2);
+  if (n_sm <= 0 || n_pairs < 2LL * n_sm || NKB > 0xFFFF) return t;
+  const int max_parts = NKB / kMinPartBlocks;                 // a dense row's key blocks allow this many parts
+  const long long rounds = n_pairs / n_sm, rem = n_pairs % n_sm;
+  if (rem == 0) return t;
+  long long best_num = 1, best_den = 1;                       // length of the last round: num / den
+  for (int parts = 2; parts <= 4 && parts <= max_parts; parts *= 2) {
+    const long long num = (rem * parts + n_sm - 1) / n_sm;    // rounds of 1/parts each
+    if (num * best_den < best_num * parts) {
+      best_num = num;
+      best_den = parts;
+      t.parts = parts;
+    }
+  }
+  // worth it from 3% of the launch on (the parts cost a fourth launch and ~4 key blocks' time each)
+  if (t.parts && (best_den - best_num) * 100 < 3 * best_den * (rounds + 1)) t.parts = 0;
+  if (t.parts) t.rem = static_cast<int>(rem);
+  return t;
 }
 
-FwdWorkspace carve_fwd_workspace(void* ws, int B, int H, int NQB) {
+static size_t al256(size_t x) { return (x + 255) / 256 * 256; }
+
+size_t fwd_workspace_bytes(int B, int H, int NQB, int W, TailPlan plan) {
+  const size_t BH = static_cast<size_t>(B) * H;
+  // two int4 arrays of BH*NQB records (+ alignment), then the parts' task list and results
+  const size_t words = 20 + 4 * BH + 8 * BH * static_cast<size_t>(NQB);
+  const size_t slots = static_cast<size_t>(plan.rem) * plan.parts;
+  return al256(words * sizeof(int32_t)) + al256(static_cast<size_t>(plan.rem) * sizeof(int4)) +
+         al256(slots * 2 * W * sizeof(uint32_t)) +
+         al256(slots * 2 * 128 * 128 * sizeof(__nv_bfloat16)) + al256(slots * 2 * 128 * sizeof(float));
+}
+
+FwdWorkspace carve_fwd_workspace(void* ws, int B, int H, int NQB, int W, TailPlan plan) {
   const size_t BH = static_cast<size_t>(B) * H;
   int32_t* p = static_cast<int32_t*>(ws);
   FwdWorkspace w;
@@ -36,17 +80,29 @@ FwdWorkspace carve_fwd_workspace(void* ws, int B, int H, int NQB) {
   w.stats = p + 2;
   w.head_cost = p + 16;
   w.head_count = w.head_cost + BH;
-  w.kmax2 = reinterpret_cast<float*>(w.head_count + BH);
-  int32_t* rec = w.head_count + 2 * BH;
-  rec += (reinterpret_cast<uintptr_t>(rec) & 7u) ? 1 : 0;                 // int2 alignment (ws is 16 B aligned)
-  w.local_items = reinterpret_cast<int2*>(rec);
+  w.head_tail = w.head_count + BH;
+  w.kmax2 = reinterpret_cast<float*>(w.head_tail + BH);
+  int32_t* rec = w.head_tail + 2 * BH;
+  rec += (4 - ((rec - p) & 3)) & 3;                                       // int4 alignment (ws is 16 B aligned)
+  w.local_items = reinterpret_cast<int4*>(rec);
   w.items = w.local_items + BH * static_cast<size_t>(NQB);
+  const size_t words = 20 + 4 * BH + 8 * BH * static_cast<size_t>(NQB);
+  char* c = static_cast<char*>(ws) + al256(words * sizeof(int32_t));
+  const size_t slots = static_cast<size_t>(plan.rem) * plan.parts;
+  w.tasks = reinterpret_cast<int4*>(c);
+  c += al256(static_cast<size_t>(plan.rem) * sizeof(int4));
+  w.part_mask = reinterpret_cast<uint32_t*>(c);
+  c += al256(slots * 2 * W * sizeof(uint32_t));
+  w.part_out = reinterpret_cast<__nv_bfloat16*>(c);
+  c += al256(slots * 2 * 128 * 128 * sizeof(__nv_bfloat16));
+  w.part_lse = reinterpret_cast<float*>(c);
   return w;
 }
 
 namespace {
 
 constexpr int kSortThreads = 1024;
+constexpr int kMaxTail = 128;             // rows-in-parts of one (b,h) group (fwd_tail_plan: <= n_sm per launch)
 constexpr uint32_t kIdxBits = 14, kIdxMask = (1u << kIdxBits) - 1u;       // rows / slots < 16384
 
 // The key-norm pass reads every key of a (b,h) group once (N * 256 B) to save ~6% of the group's
@@ -106,13 +162,17 @@ __device__ __forceinline__ int pow2_at_least(int n) {
 
 
 // grid = B*H blocks. Builds the items of group (b,h), sorted by cost (active tiles) descending:
-// local_items[bh][pos] = {cost, ua | ub << 16} (ub = 0xFFFF: single-row item); head_cost[bh] =
-// active tiles of the group; head_count[bh] = its number of items.
+// local_items[bh][pos] = {cost, ua | ub << 16, part slot or -1, 0} (ub =
+// 0xFFFF: single-row item); head_cost[bh] = active tiles of the group; head_count[bh] = its number
+// of items, the last head_tail[bh] of which (the parts of the group's lightest items, plan.rem of
+// them over all groups) belong at the end of the issue order; tasks[] lists the rows issued in parts.
 // Dynamic shared memory: keys[n2] (uint32), then pop[NQB], ia[slots], ib[slots] (uint16).
 __global__ void __launch_bounds__(kSortThreads)
 schedule_items_kernel(const uint32_t* __restrict__ mask_bits, int H, int NQB, int NKB, int W,
-                      int pair_rows, int split_rows, int n2, int32_t* __restrict__ head_cost,
-                      int32_t* __restrict__ head_count, int2* __restrict__ local_items,
+                      int pair_rows, int split_rows, int plan_rem, int plan_parts, int n2,
+                      int32_t* __restrict__ head_cost, int32_t* __restrict__ head_count,
+                      int32_t* __restrict__ head_tail, int4* __restrict__ local_items,
+                      int4* __restrict__ tasks, uint32_t* __restrict__ part_mask,
                       float* __restrict__ kmax2) {
   extern __shared__ uint32_t s_dyn[];
   const int slots = NQB + 2;
@@ -253,18 +313,118 @@ schedule_items_kernel(const uint32_t* __restrict__ mask_bits, int H, int NQB, in
   __syncthreads();
   sort_desc(s_keys, s_alt, min(used, slots), n2);
   const int count = s_count;
-  for (int pos = threadIdx.x; pos < count; pos += blockDim.x) {
+  // this group's share of the plan's rows-in-parts: tasks [t0, t0 + n_tail) of plan_rem
+  const long long BH = static_cast<long long>(gridDim.x);
+  const int t0 = static_cast<int>(bh * static_cast<long long>(plan_rem) / BH);
+  const int t1 = static_cast<int>((bh + 1) * static_cast<long long>(plan_rem) / BH);
+  // (the group's record arrays hold NQB entries: count + n_tail * (parts - 1) must fit)
+  const int n_tail = min(min(min(t1 - t0, count), kMaxTail),
+                         plan_parts > 1 ? (NQB - count) / (plan_parts - 1) : 0);
+  const int n_main = count - n_tail;
+  for (int k = n_tail + threadIdx.x; k < t1 - t0; k += blockDim.x) tasks[t0 + k] = make_int4(-1, 0, 0, 0);
+  for (int pos = threadIdx.x; pos < n_main; pos += blockDim.x) {
     const uint32_t key = s_keys[pos];
     const int s = static_cast<int>(kIdxMask - (key & kIdxMask));
     // single-row items of the tcgen05 kernel are SPLIT items (ub = ua): the row's key blocks go to
     // the kernel's two tiles in turn, so both softmax warpgroups work on the one row
     const int ub = (!pair_rows && split_rows) ? s_a[s] : s_b[s];
     local_items[static_cast<size_t>(bh) * NQB + pos] =
-        make_int2(static_cast<int>(key >> kIdxBits) - 1, s_a[s] | (ub << 16));
+        make_int4(static_cast<int>(key >> kIdxBits) - 1, s_a[s] | (ub << 16), -1, 0);
+  }
+  // ---- the group's lightest items, in parts. One warp per item: the union of its bit-rows is cut
+  // where its key blocks' running count passes c * i / parts (items of fewer than kMinPartBlocks key
+  // blocks per part take fewer parts, or stay whole)
+  __shared__ int s_np[kMaxTail], s_cut[kMaxTail][3], s_at[kMaxTail + 1];
+  for (int k = warp; k < n_tail; k += kSortThreads / 32) {
+    const int s = static_cast<int>(kIdxMask - (s_keys[n_main + k] & kIdxMask));
+    const int a = s_a[s], b = s_b[s];
+    const uint32_t* ma = rows + static_cast<size_t>(a) * W;
+    const uint32_t* mb = (b != 0xFFFF && b != a) ? rows + static_cast<size_t>(b) * W : ma;
+    int c = 0;
+    for (int w = lane; w < W; w += 32) {
+      const uint32_t keep = (w == W - 1) ? tail_mask : 0xFFFFFFFFu;
+      c += __popc((__ldg(ma + w) | __ldg(mb + w)) & keep);
+    }
+    c = __reduce_add_sync(0xFFFFFFFFu, c);
+    int np = plan_parts;
+    while (np > 1 && c < kMinPartBlocks * np) np >>= 1;
+    // key block holding the union's bit of rank r_i = c * i / np: part i starts there
+    int done = 0, next = 1;
+    for (int w0 = 0; w0 < W && next < np; w0 += 32) {
+      const int w = w0 + lane;
+      uint32_t x = 0u;
+      if (w < W) x = (__ldg(ma + w) | __ldg(mb + w)) & ((w == W - 1) ? tail_mask : 0xFFFFFFFFu);
+      const int n = __popc(x);
+      int incl = n;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+        if (lane >= o) incl += v;
+      }
+      const int chunk = __shfl_sync(0xFFFFFFFFu, incl, 31);
+      while (next < np) {
+        const int r = static_cast<int>(static_cast<long long>(c) * next / np) - done;   // rank inside this chunk
+        if (r >= chunk) break;
+        const bool mine = r >= incl - n && r < incl;
+        const uint32_t who = __ballot_sync(0xFFFFFFFFu, mine);
+        const int bit = mine ? static_cast<int>(__fns(x, 0, r - (incl - n) + 1)) : 0;
+        const int kb = __shfl_sync(0xFFFFFFFFu, w * 32 + bit, __ffs(who) - 1);
+        if (lane == 0) s_cut[k][next - 1] = kb;
+        ++next;
+      }
+      done += chunk;
+    }
+    if (lane == 0) s_np[k] = np;
+  }
+  __syncthreads();
+  // items that stay whole keep their place in the group's list (their K/V is in L2 while the group
+  // runs); only real parts move to the end of the issue order
+  __shared__ int s_main_end;
+  if (threadIdx.x == 0) {
+    int at = n_main;
+    for (int k = 0; k < n_tail; ++k)
+      if (s_np[k] == 1) s_at[k] = at++;
+    s_main_end = at;
+    for (int k = 0; k < n_tail; ++k)
+      if (s_np[k] > 1) {
+        s_at[k] = at;
+        at += s_np[k];
+      }
+    s_at[n_tail] = at;
+  }
+  __syncthreads();
+  for (int k = warp; k < n_tail; k += kSortThreads / 32) {
+    const uint32_t key = s_keys[n_main + k];
+    const int s = static_cast<int>(kIdxMask - (key & kIdxMask));
+    const int rows_ab = s_a[s] | (s_b[s] << 16);
+    const int np = s_np[k], slot0 = (t0 + k) * plan_parts;
+    if (lane < np)
+      local_items[static_cast<size_t>(bh) * NQB + s_at[k] + lane] =
+          make_int4(static_cast<int>(key >> kIdxBits) - 1, rows_ab, np > 1 ? slot0 + lane : -1, 0);
+    if (np > 1) {
+      // the parts' bit-rows: rows a and b with the bits of part i's key range [lo_i, hi_i) only
+      const int a = rows_ab & 0xFFFF, b = (rows_ab >> 16) & 0xFFFF;
+      const uint32_t* ma = rows + static_cast<size_t>(a) * W;
+      const uint32_t* mb = rows + static_cast<size_t>(b != 0xFFFF ? b : a) * W;
+      for (int i = 0; i < np; ++i) {
+        const int lo = i == 0 ? 0 : s_cut[k][i - 1];
+        const int hi = i == np - 1 ? 32 * W : s_cut[k][i];
+        uint32_t* dst = part_mask + static_cast<size_t>(2 * (slot0 + i)) * W;
+        for (int w = lane; w < W; w += 32) {
+          const int l = max(lo - 32 * w, 0), h2 = min(hi - 32 * w, 32);
+          const uint32_t m = l < h2 ? (0xFFFFFFFFu << l) & (0xFFFFFFFFu >> (32 - h2)) : 0u;
+          dst[w] = __ldg(ma + w) & m;
+          dst[W + w] = __ldg(mb + w) & m;
+        }
+      }
+    }
+    if (lane == 0) tasks[t0 + k] = make_int4(np > 1 ? bh : -1, rows_ab, np, slot0);
   }
   if (threadIdx.x == 0) {
+    const int at = s_at[n_tail];
     head_cost[bh] = s_total;
-    head_count[bh] = count;
+    head_count[bh] = at;
+    head_tail[bh] = at - s_main_end;
     // the key-norm pass (next on the stream) takes the max into kmax2[bh] -- or skips the group and
     // leaves the "no bound" mark when it is too sparse for the pass to pay (key_norm_wanted)
     kmax2[bh] = key_norm_wanted(s_total, NKB) ? 0.f : -1.f;
@@ -311,36 +471,49 @@ __device__ __forceinline__ void key_norm_slice(const __nv_bfloat16* __restrict__
 // kmax2[bh] (one launch instead of two: the forward call is launch-latency bound on short sequences).
 __global__ void __launch_bounds__(kFlatThreads)
 schedule_flatten_kernel(const int32_t* __restrict__ head_cost, const int32_t* __restrict__ head_count,
-                        const int2* __restrict__ local_items, int BH, int NQB, int flatten,
-                        int2* __restrict__ items, int32_t* __restrict__ cursor,
+                        const int32_t* __restrict__ head_tail, const int4* __restrict__ local_items,
+                        int BH, int NQB, int flatten,
+                        int4* __restrict__ items, int32_t* __restrict__ cursor,
                         int32_t* __restrict__ n_items, const __nv_bfloat16* __restrict__ k, int N,
                         int n_valid, float* __restrict__ kmax2) {
   const int bh = blockIdx.y;
+  griddep_wait();
   if (flatten) {
     const int count = __ldg(head_count + bh);
     const bool first = blockIdx.x == 0 && bh == 0;
     if (static_cast<int>(blockIdx.x) * kFlatThreads < count || first) {
-      __shared__ int s_start, s_all;
-      if (threadIdx.x == 0) s_start = s_all = 0;
+      // main part of the order: every group's items but its tail; then the groups' tails
+      __shared__ int s_start, s_tstart, s_all, s_tall;
+      if (threadIdx.x == 0) s_start = s_tstart = s_all = s_tall = 0;
       __syncthreads();
       const int cg = __ldg(head_cost + bh);
-      int start = 0, all = 0;
+      int start = 0, tstart = 0, all = 0, tall = 0;
       for (int j = threadIdx.x; j < BH; j += kFlatThreads) {
-        const int cj = __ldg(head_cost + j), nj = __ldg(head_count + j);
+        const int cj = __ldg(head_cost + j), nj = __ldg(head_count + j), tj = __ldg(head_tail + j);
         all += nj;
-        if (cj > cg || (cj == cg && j < bh)) start += nj;
+        tall += tj;
+        if (cj > cg || (cj == cg && j < bh)) {
+          start += nj - tj;
+          tstart += tj;
+        }
       }
       start = __reduce_add_sync(0xFFFFFFFFu, start);
+      tstart = __reduce_add_sync(0xFFFFFFFFu, tstart);
       all = __reduce_add_sync(0xFFFFFFFFu, all);
+      tall = __reduce_add_sync(0xFFFFFFFFu, tall);
       if ((threadIdx.x & 31) == 0) {
         atomicAdd(&s_start, start);
+        atomicAdd(&s_tstart, tstart);
         atomicAdd(&s_all, all);
+        atomicAdd(&s_tall, tall);
       }
       __syncthreads();
       const int pos = blockIdx.x * kFlatThreads + threadIdx.x;
       if (pos < count) {
-        const int2 rec = __ldg(local_items + static_cast<size_t>(bh) * NQB + pos);
-        items[s_start + pos] = make_int2(bh, rec.y);
+        const int4 rec = __ldg(local_items + static_cast<size_t>(bh) * NQB + pos);
+        const int n_main = count - __ldg(head_tail + bh);
+        const int at = pos < n_main ? s_start + pos : (s_all - s_tall) + s_tstart + (pos - n_main);
+        items[at] = make_int4(bh, rec.y, rec.z, 0);
       }
       if (first && threadIdx.x == 0) {
         cursor[0] = 0;
@@ -360,6 +533,72 @@ schedule_flatten_kernel(const int32_t* __restrict__ head_cost, const int32_t* __
   }
 }
 
+// grid = (plan.rem, 2), 256 threads: block (t, tile) merges the parts of query block ua (tile 0) / ub
+// (tile 1) of task t. A part holds the softmax over its key range: normalised O_i (bf16) and lse_i;
+// over the whole row  lse = m + ln sum_i e^(lse_i - m),  O = sum_i e^(lse_i - lse) O_i, summed in part
+// order. A warp takes 16 rows, row by row across the 256 bytes of a row (8 bytes per lane), four rows'
+// loads in flight; lane r holds the weights of the warp's row r. Launched with programmatic stream
+// serialization: the launch overlaps the attention kernel, griddepcontrol.wait orders the reads.
+__global__ void __launch_bounds__(256)
+combine_parts_kernel(const int4* __restrict__ tasks, const __nv_bfloat16* __restrict__ part_out,
+                     const float* __restrict__ part_lse, int N, __nv_bfloat16* __restrict__ out,
+                     float* __restrict__ lse) {
+  griddep_wait();
+  const int4 task = __ldg(tasks + blockIdx.x);              // {b*H + h, ua | ub << 16, parts, first slot}
+  const int tile = blockIdx.y;
+  const int ua = task.y & 0xFFFF, ub = (task.y >> 16) & 0xFFFF;
+  if (task.x < 0 || (tile == 1 && (ub == 0xFFFF || ub == ua))) return;   // whole item / one row only
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int np = task.z;
+  const int row = warp * 16 + (lane & 15);                  // lanes 16-31 mirror 0-15
+  float l[4], m = -INFINITY;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    l[i] = i < np ? __ldcg(part_lse + (static_cast<size_t>(2 * (task.w + i) + tile) * 128 + row)) : -INFINITY;
+    m = fmaxf(m, l[i]);
+  }
+  float wgt[4], sum = 0.f;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    wgt[i] = l[i] > -INFINITY ? expf(l[i] - m) : 0.f;
+    sum += wgt[i];
+  }
+  const float inv = sum > 0.f ? 1.f / sum : 0.f;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) wgt[i] *= inv;
+  const size_t grow0 = static_cast<size_t>(task.x) * N + static_cast<size_t>(tile == 0 ? ua : ub) * 128 + warp * 16;
+  if (lane < 16) lse[grow0 + lane] = sum > 0.f ? m + logf(sum) : -INFINITY;
+#pragma unroll 1
+  for (int r0 = 0; r0 < 16; r0 += 4) {
+    uint2 x[4][4];
+#pragma unroll
+    for (int rr = 0; rr < 4; ++rr)
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+        if (i < np)
+          x[rr][i] = __ldcg(reinterpret_cast<const uint2*>(
+                                part_out + (static_cast<size_t>(2 * (task.w + i) + tile) * 128 + warp * 16 + r0 + rr) * 128) +
+                            lane);
+#pragma unroll
+    for (int rr = 0; rr < 4; ++rr) {
+      float acc[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const float sc = __shfl_sync(0xFFFFFFFFu, wgt[i], r0 + rr);
+        if (i < np) {
+          acc[0] = fmaf(__uint_as_float(x[rr][i].x << 16), sc, acc[0]);
+          acc[1] = fmaf(__uint_as_float(x[rr][i].x & 0xFFFF0000u), sc, acc[1]);
+          acc[2] = fmaf(__uint_as_float(x[rr][i].y << 16), sc, acc[2]);
+          acc[3] = fmaf(__uint_as_float(x[rr][i].y & 0xFFFF0000u), sc, acc[3]);
+        }
+      }
+      const __nv_bfloat162 lo = __floats2bfloat162_rn(acc[0], acc[1]), hi = __floats2bfloat162_rn(acc[2], acc[3]);
+      reinterpret_cast<uint2*>(out + (grow0 + r0 + rr) * 128)[lane] =
+          make_uint2(*reinterpret_cast<const uint32_t*>(&lo), *reinterpret_cast<const uint32_t*>(&hi));
+    }
+  }
+}
+
 __global__ void __launch_bounds__(128)
 enumerate_kernel(const uint32_t* __restrict__ mask_bits, int rows, int NKB, int W,
                  int32_t* __restrict__ idx, int32_t* __restrict__ cnt) {
@@ -375,8 +614,8 @@ enumerate_kernel(const uint32_t* __restrict__ mask_bits, int rows, int NKB, int 
 
 }  // namespace
 
-cudaError_t launch_schedule(const FwdParams& p, const FwdWorkspace& w, int rpi, cudaStream_t st,
-                            int* n_launch, bool reuse) {
+cudaError_t launch_schedule(const FwdParams& p, const FwdWorkspace& w, int rpi, TailPlan plan,
+                            cudaStream_t st, int* n_launch, bool reuse) {
   const int BH = p.B * p.H;
   const bool norms = p.D == 128 && p.kmax2 != nullptr;   // the tcgen05 kernel's score bound needs max |k|^2
   cudaError_t e;
@@ -397,19 +636,37 @@ cudaError_t launch_schedule(const FwdParams& p, const FwdWorkspace& w, int rpi, 
       if (e != cudaSuccess) return e;
     }
     schedule_items_kernel<<<BH, kSortThreads, smem, st>>>(p.mask_bits, p.H, p.NQB, p.NKB, p.W, rpi == 2 ? 1 : 0,
-                                                         p.split_rows, n2, w.head_cost, w.head_count,
-                                                         w.local_items, w.kmax2);
+                                                         p.split_rows, rpi == 2 ? plan.rem : 0, plan.parts, n2,
+                                                         w.head_cost, w.head_count, w.head_tail, w.local_items,
+                                                         w.tasks, w.part_mask, w.kmax2);
     *n_launch += 1;
   }
   if (!reuse || norms) {
     const int xf = reuse ? 0 : (p.NQB + kFlatThreads - 1) / kFlatThreads;
     const int xn = norms ? (p.n_valid + kNormRowsPerBlock - 1) / kNormRowsPerBlock : 0;
     const dim3 grid(xf > xn ? xf : xn, BH);
-    schedule_flatten_kernel<<<grid, kFlatThreads, 0, st>>>(w.head_cost, w.head_count, w.local_items, BH, p.NQB,
-                                                          reuse ? 0 : 1, w.items, w.cursor, w.n_items,
-                                                          norms ? p.k : nullptr, p.N, p.n_valid, w.kmax2);
+    const int32_t* hc = w.head_cost;
+    const int32_t* hn = w.head_count;
+    const int32_t* ht = w.head_tail;
+    const int4* li = w.local_items;
+    e = launch_pdl(schedule_flatten_kernel, grid, dim3(kFlatThreads), 0, st, hc, hn, ht, li, BH, p.NQB,
+                   reuse ? 0 : 1, w.items, w.cursor, w.n_items, norms ? p.k : nullptr, p.N, p.n_valid, w.kmax2);
+    if (e != cudaSuccess) return e;
     *n_launch += 1;
   }
+  return cudaGetLastError();
+}
+
+cudaError_t launch_combine_parts(const FwdParams& p, const FwdWorkspace& w, TailPlan plan,
+                                 cudaStream_t st, int* n_launch) {
+  if (plan.rem <= 0) return cudaSuccess;
+  const int4* tasks = w.tasks;
+  const __nv_bfloat16* po = w.part_out;
+  const float* pl = w.part_lse;
+  cudaError_t e = launch_pdl(combine_parts_kernel, dim3(plan.rem, 2), dim3(256), 0, st, tasks, po, pl, p.N, p.out,
+                             p.lse);
+  if (e != cudaSuccess) return e;
+  *n_launch += 1;
   return cudaGetLastError();
 }
 

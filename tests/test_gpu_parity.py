@@ -192,6 +192,56 @@ def test_pack_mask_bit_exact_adversarial_scores(sa, NQB, NKB, force_diag):
         assert dense[h].sum() == oracle.keep_count(density[h], NQB, NKB, force_diag)
 
 
+@pytest.mark.parametrize("H,NQB,NKB,force_diag", [(1, 700, 700, 1), (3, 1, 1, 1), (2, 1, 3, 0), (5, 3, 2, 1),
+                                                  (1300, 9, 7, 1), (2, 300, 301, 1), (2, 301, 300, 0)])
+def test_pack_mask_special_values_and_block_runs(sa, H, NQB, NKB, force_diag):
+    # the histogram blocks take flat runs of a head's entries (several runs per head at 700 x 700,
+    # one run per head at H = 1300, runs that start off a 16-byte boundary whenever NQB * NKB is odd)
+    # and treat the forced diagonal as a correction: signed zeros, denormals and huge values sit on
+    # and off the diagonal, and a head has ties exactly at the threshold
+    rng = np.random.Generator(np.random.PCG64(H * 7919 + NQB * 31 + NKB))
+    scores = (rng.standard_normal((H, NQB, NKB)) * rng.choice([1e-40, 1e-3, 1.0, 1e30], size=(H, 1, 1))
+              ).astype(np.float32)
+    special = np.asarray([0.0, -0.0, 1e-45, -1e-45, 3.4e38, -3.4e38, 1.0, -1.0], dtype=np.float32)
+    hit = rng.random(scores.shape) < 0.05
+    scores[hit] = rng.choice(special, size=int(hit.sum()))
+    for h in range(H):
+        for u in range(min(NQB, NKB)):
+            if (h + u) % 5 == 0:
+                scores[h, u, u] = special[(h + u) % len(special)]
+    if H > 1:
+        scores[1] = np.round(np.clip(scores[1], -100.0, 100.0) * 2) / 2     # ties at the threshold
+    density = rng.uniform(0.01, 1.0, size=H).astype(np.float32)
+    got, want = _pack_both(sa, scores, density, force_diag)
+    assert (got == want).all()
+
+
+def test_pack_mask_non_finite_scores_follow_the_documented_order(sa):
+    # outside the oracle's domain (it takes finite scores): include/scalingattn.h orders NaN lowest,
+    # then -inf .. +inf with -0 == +0, ties by flat index. Checked as properties of the result.
+    rng = np.random.Generator(np.random.PCG64(5))
+    H, NQB, NKB = 4, 70, 90
+    scores = rng.standard_normal((H, NQB, NKB)).astype(np.float32)
+    special = np.asarray([np.nan, np.inf, -np.inf, 0.0, -0.0], dtype=np.float32)
+    hit = rng.random(scores.shape) < 0.3
+    scores[hit] = rng.choice(special, size=int(hit.sum()))
+    density = np.asarray([0.05, 0.4, 0.8, 0.97], dtype=np.float32)
+    got = host_bits(sa.sa_pack_mask(torch.from_numpy(scores).cuda(), torch.from_numpy(density).cuda(),
+                                    force_diag=False))
+    kept = oracle.unpack_mask(got, NKB).astype(bool)
+    rank = np.where(np.isnan(scores), -np.inf, scores.astype(np.float64))
+    rank = np.where(np.isnan(scores), -1e300, np.where(np.isinf(rank), np.sign(rank) * 1e200, rank))
+    for h in range(H):
+        k = oracle.keep_count(density[h], NQB, NKB, 0)
+        assert kept[h].sum() == k
+        r, m = rank[h].ravel(), kept[h].ravel()
+        lo = r[m].min()
+        assert r[~m].max() <= lo                       # a top set of the order
+        tied = np.flatnonzero(r == lo)                 # ties at the threshold: first ones in flat order
+        n_tied_kept = int(m[tied].sum())
+        assert m[tied[:n_tied_kept]].all() and not m[tied[n_tied_kept:]].any()
+
+
 def test_pack_mask_extreme_densities(sa):
     rng = np.random.Generator(np.random.PCG64(77))
     scores = rng.random((3, 64, 64)).astype(np.float32)
@@ -905,6 +955,53 @@ def test_short_signature_call_on_two_streams(sa):
     o, l = sa.sa_block_sparse_attn_fwd(q.cuda(), k.cuda(), v.cuda(), bits, blk, blk, scale, stream=streams[0])
     torch.cuda.synchronize()
     assert torch.equal(o, wo) and torch.equal(l, wl)
+
+
+@pytest.mark.parametrize("H,N,n_valid,density", [(8, 9600, 9590, 0.8), (3, 25600, 25600, 0.12), (5, 16384, 16384, 1.0)])
+def test_last_round_rows_in_parts_match_oracle(sa, H, N, n_valid, density):
+    # Pair items that do not fill a whole number of rounds over the SMs (here 304 / 300 / 320 pairs on
+    # 148 SMs): the lightest rows of every head are issued in parts over key ranges (2 parts at 9600,
+    # 4 at 16384; at density 0.12 the rows are too short and stay whole) and merged by
+    # combine_parts_kernel (a 4th launch). Every row is compared with the oracle; the rows in parts
+    # differ from the pair path (variant 2) by the parts' bf16 rounding only.
+    cfg = inputs.seq_grid_config(N, H=H, n_valid=n_valid, seed=31)
+    q, k, v = inputs.make_qkv(cfg)
+    inputs.poison_padding(cfg, k, v)
+    scores, dens = inputs.iid_block_scores(cfg, density, seed=32)
+    scores[:, :, 0] += 2.0                                    # a sink column
+    scores[0, 5] += 3.0                                       # a dense row next to sparse ones
+    bits = oracle.pack_mask(scores, dens, 1)
+    out, lse = run_fwd(sa, q, k, v, bits, 128, cfg.scale, n_valid=n_valid, variant=0)
+    assert sa.sa_last_launch_count() == 4
+    out2, lse2 = run_fwd(sa, q, k, v, bits, 128, cfg.scale, n_valid=n_valid, variant=2)
+    assert sa.sa_last_launch_count() == 3
+    d = (out.float() - out2.float()).abs()
+    assert d.max().item() <= 2e-2 and (lse - lse2).abs().max().item() <= 1e-5
+    changed = (d.reshape(H, cfg.NQB, -1).amax(dim=2) > 0).sum().item()
+    if density < 0.5:
+        assert changed == 0                                   # rows too short for parts: the same bits
+    else:
+        assert 0 < changed <= 2 * 148                         # only the rows of the last round
+    if density < 1.0:
+        ref_o, ref_l = oracle.attn(inputs.as_u16(q), inputs.as_u16(k), inputs.as_u16(v), bits, 128, 128,
+                                   cfg.scale, n_valid=n_valid)
+        check_out(out, lse, ref_o, ref_l, "rows in parts")
+    else:                                                     # dense: the oracle on two heads' worth of sampled rows
+        units = [(0, h, u) for h in (0, H - 1) for u in (0, 1, cfg.NQB - 2, cfg.NQB - 1)]
+        ref_o, ref_l = oracle.attn_units(inputs.as_u16(q), inputs.as_u16(k), inputs.as_u16(v), bits, units, 128,
+                                         128, cfg.scale, n_valid=n_valid)
+        for i, (b, h, u) in enumerate(units):
+            check_out(out[b, h, u * 128:(u + 1) * 128], lse[b, h, u * 128:(u + 1) * 128], ref_o[i], ref_l[i],
+                      f"unit {h},{u}")
+    # run to run, and through the schedule-reuse form: the same bits
+    ws = torch.empty(sa.sa_fwd_workspace_bytes(1, H, N, 128), dtype=torch.uint8, device="cuda")
+    a_o, a_l = sa.sa_block_sparse_attn_fwd_ex(q.cuda(), k.cuda(), v.cuda(), dev_bits(bits), 128, 128, cfg.scale,
+                                              n_valid=n_valid, workspace=ws)
+    b_o, b_l = sa.sa_block_sparse_attn_fwd_ex(q.cuda(), k.cuda(), v.cuda(), dev_bits(bits), 128, 128, cfg.scale,
+                                              n_valid=n_valid, workspace=ws, reuse_schedule=True)
+    torch.cuda.synchronize()
+    assert torch.equal(a_o, out) and torch.equal(a_l, lse) and torch.equal(b_o, out) and torch.equal(b_l, lse)
+
 
 
 def test_cuda_library_is_the_path(sa):
