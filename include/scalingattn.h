@@ -156,7 +156,12 @@ SA_API sa_status sa_block_sparse_attn_fwd(const void* q, const void* k, const vo
 
 /* Same, plus n_valid (keys >= n_valid get exactly zero weight, even inside an active block; query
  * rows >= n_valid are computed like any other row) and a caller-provided workspace of at least
- * sa_fwd_workspace_bytes(B,H,N,Bq) bytes (16 B aligned), so nothing is allocated in the call. */
+ * sa_fwd_workspace_bytes(B,H,N,Bq) bytes (16 B aligned), so nothing is allocated in the call.
+ * sa_fwd_workspace_bytes is for the CURRENT device: besides the work list the workspace holds the
+ * partial results of the query blocks that a call issues in parts over key ranges (the partly filled
+ * last round of work items over the device's SMs; merged by one more kernel of the same call), whose
+ * number depends on the SM count. Deterministic: a given (shape, mask, SM count) always takes the same
+ * parts, merged in a fixed order. 3 or 4 kernels on `stream`. */
 SA_API sa_status sa_block_sparse_attn_fwd_ex(const void* q, const void* k, const void* v,
                                       const uint32_t* mask_bits, void* out, float* lse, int B,
                                       int H, int N, int n_valid, int D, int Bq, int Bk,
@@ -167,8 +172,9 @@ SA_API sa_status sa_block_sparse_attn_fwd_ex(const void* q, const void* k, const
  * per layer, timestep and head and reused by every call): same as sa_block_sparse_attn_fwd_ex, but the
  * work list that an earlier _ex call left in `workspace` is reused instead of being rebuilt, so the
  * two schedule kernels are skipped (their ~14 us matter at short sequences). Precondition: `workspace`
- * was last filled by sa_block_sparse_attn_fwd_ex (or this call) with the same B, H, N, Bq, Bk, the same
- * forward variant and a mask with the same contents; the result is undefined otherwise. */
+ * was last filled by sa_block_sparse_attn_fwd_ex (or this call) on the same device with the same B, H,
+ * N, Bq, Bk, the same forward variant and a mask with the same contents; the result is undefined
+ * otherwise. */
 SA_API sa_status sa_block_sparse_attn_fwd_reuse(const void* q, const void* k, const void* v,
                                          const uint32_t* mask_bits, void* out, float* lse, int B,
                                          int H, int N, int n_valid, int D, int Bq, int Bk,
