@@ -313,6 +313,22 @@ schedule_items_kernel(const uint32_t* __restrict__ mask_bits, int H, int NQB, in
   __syncthreads();
   sort_desc(s_keys, s_alt, min(used, slots), n2);
   const int count = s_count;
+  // HEAVY items: at least four times the group's mean item and 64 key blocks (BASELINE.json's
+  // adversarial mask: the pairs of fully dense rows next to diagonal-only ones). They lead the
+  // sorted list; the issue order takes the heavy items of ALL groups first, so that the launch does
+  // not end on the last group's long items while the other SMs have run out of work.
+  __shared__ int s_heavy;
+  if (threadIdx.x == 0) s_heavy = 0;
+  __syncthreads();
+  {
+    int mine_heavy = 0;
+    for (int pos = threadIdx.x; pos < count; pos += blockDim.x) {
+      const long long cost = static_cast<long long>(s_keys[pos] >> kIdxBits) - 1;
+      mine_heavy += (cost >= 64 && cost * count >= 4LL * s_total) ? 1 : 0;
+    }
+    if (mine_heavy) atomicAdd(&s_heavy, mine_heavy);
+  }
+  __syncthreads();
   // this group's share of the plan's rows-in-parts: tasks [t0, t0 + n_tail) of plan_rem
   const long long BH = static_cast<long long>(gridDim.x);
   const int t0 = static_cast<int>(bh * static_cast<long long>(plan_rem) / BH);
@@ -424,7 +440,7 @@ schedule_items_kernel(const uint32_t* __restrict__ mask_bits, int H, int NQB, in
     const int at = s_at[n_tail];
     head_cost[bh] = s_total;
     head_count[bh] = at;
-    head_tail[bh] = at - s_main_end;
+    head_tail[bh] = (at - s_main_end) | (min(s_heavy, n_main) << 16);
     // the key-norm pass (next on the stream) takes the max into kmax2[bh] -- or skips the group and
     // leaves the "no bound" mark when it is too sparse for the pass to pay (key_norm_wanted)
     kmax2[bh] = key_norm_wanted(s_total, NKB) ? 0.f : -1.f;
@@ -482,39 +498,44 @@ schedule_flatten_kernel(const int32_t* __restrict__ head_cost, const int32_t* __
     const int count = __ldg(head_count + bh);
     const bool first = blockIdx.x == 0 && bh == 0;
     if (static_cast<int>(blockIdx.x) * kFlatThreads < count || first) {
-      // main part of the order: every group's items but its tail; then the groups' tails
-      __shared__ int s_start, s_tstart, s_all, s_tall;
-      if (threadIdx.x == 0) s_start = s_tstart = s_all = s_tall = 0;
+      // the order: every group's HEAVY items (head_tail >> 16 of them, the first of its list), then
+      // every group's other whole items, then the groups' parts (head_tail & 0xFFFF, the last of its list)
+      __shared__ int s_sum[6];        // items / heavy / tail: of the groups ahead, of all groups
+      if (threadIdx.x < 6) s_sum[threadIdx.x] = 0;
       __syncthreads();
       const int cg = __ldg(head_cost + bh);
-      int start = 0, tstart = 0, all = 0, tall = 0;
+      int v[6] = {0, 0, 0, 0, 0, 0};
       for (int j = threadIdx.x; j < BH; j += kFlatThreads) {
-        const int cj = __ldg(head_cost + j), nj = __ldg(head_count + j), tj = __ldg(head_tail + j);
-        all += nj;
-        tall += tj;
+        const int cj = __ldg(head_cost + j), nj = __ldg(head_count + j), pj = __ldg(head_tail + j);
+        const int hj = pj >> 16, tj = pj & 0xFFFF;
+        v[3] += nj;
+        v[4] += hj;
+        v[5] += tj;
         if (cj > cg || (cj == cg && j < bh)) {
-          start += nj - tj;
-          tstart += tj;
+          v[0] += nj;
+          v[1] += hj;
+          v[2] += tj;
         }
       }
-      start = __reduce_add_sync(0xFFFFFFFFu, start);
-      tstart = __reduce_add_sync(0xFFFFFFFFu, tstart);
-      all = __reduce_add_sync(0xFFFFFFFFu, all);
-      tall = __reduce_add_sync(0xFFFFFFFFu, tall);
-      if ((threadIdx.x & 31) == 0) {
-        atomicAdd(&s_start, start);
-        atomicAdd(&s_tstart, tstart);
-        atomicAdd(&s_all, all);
-        atomicAdd(&s_tall, tall);
+#pragma unroll
+      for (int i = 0; i < 6; ++i) {
+        v[i] = __reduce_add_sync(0xFFFFFFFFu, v[i]);
+        if ((threadIdx.x & 31) == 0 && v[i]) atomicAdd(&s_sum[i], v[i]);
       }
       __syncthreads();
       const int pos = blockIdx.x * kFlatThreads + threadIdx.x;
       if (pos < count) {
         const int4 rec = __ldg(local_items + static_cast<size_t>(bh) * NQB + pos);
-        const int n_main = count - __ldg(head_tail + bh);
-        const int at = pos < n_main ? s_start + pos : (s_all - s_tall) + s_tstart + (pos - n_main);
+        const int packed = __ldg(head_tail + bh);
+        const int n_heavy = packed >> 16, n_main = count - (packed & 0xFFFF);
+        const int all = s_sum[3], all_heavy = s_sum[4], all_tail = s_sum[5];
+        int at;
+        if (pos < n_heavy) at = s_sum[1] + pos;
+        else if (pos < n_main) at = all_heavy + (s_sum[0] - s_sum[1] - s_sum[2]) + (pos - n_heavy);
+        else at = (all - all_tail) + s_sum[2] + (pos - n_main);
         items[at] = make_int4(bh, rec.y, rec.z, 0);
       }
+      const int s_all = s_sum[3];
       if (first && threadIdx.x == 0) {
         cursor[0] = 0;
         cursor[2] = cursor[3] = 0;    // softmax-path counters of the coming call
