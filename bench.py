@@ -546,11 +546,15 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> int:
     tb = qh.numel() * 2
     h2d = 3 * tb + scores_h.numel() * 4 + density_h.numel() * 4
     d2h = tb + lse_h.numel() * 4 + bits_h.numel() * 4
-    # the e2e result equals the device-resident one (same kernels, same inputs)
+    # the e2e result against the device-resident one (same kernels, same inputs). The host form runs
+    # head group by head group, and a group's last round of work items may be cut into parts where
+    # the whole problem's is not (K2): those rows then differ by the parts' bf16 rounding.
     same = bool(torch.equal(out_h, out.cpu()) and torch.equal(bits_h, bits.cpu()))
+    e2e_max_diff = float((out_h.float() - out.cpu().float()).abs().max())
+    assert torch.equal(bits_h, bits.cpu()) and e2e_max_diff <= 2e-2, e2e_max_diff
     del scratch
     log(f"[bench] e2e leg: {e2e_ms_local:.1f} ms/step ({h2d / 1e9:.2f} GB in, {d2h / 1e9:.2f} GB "
-        f"out), result identical to device leg: {same}")
+        f"out), result identical to device leg: {same} (max abs diff {e2e_max_diff:.3g})")
 
     # ---- density sweep at the same shapes (BASELINE.json config 4): speedup vs density 1
     sweep = []
@@ -761,7 +765,8 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> int:
                             "peaks": peaks["source"]},
             "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms, "steps": e2e_steps,
                     "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "api": "sa_hot_path_host", "matches_device_leg": same},
+                    "api": "sa_hot_path_host", "matches_device_leg": same,
+                    "max_abs_diff_vs_device_leg": e2e_max_diff},
             "gpu_launches": gpu_launches,
             "clocks": clocks,
             "softmax_path": {"warp_items_fixed_reference": path_fixed, "warp_items_exact_max": path_exact,

@@ -154,12 +154,27 @@ size_t sa_fwd_workspace_bytes(int B, int H, int N, int Bq) {
 
 static size_t al256(size_t x) { return (x + 255) / 256 * 256; }
 
+// The host forms run the forward pass head group by head group (kPipeGroups chunks per batch entry,
+// pipelined with the copies), every chunk through the same workspace: the largest chunk call's need
+// (a chunk's plan for its last round differs from the whole problem's).
+static size_t host_pipeline_ws_bytes(int H, int N, int Bq) {
+  const int groups = H < kPipeGroups ? H : kPipeGroups;
+  size_t need = 0;
+  for (int g = 0; g < groups; ++g) {
+    const int h0 = static_cast<int>(static_cast<long long>(H) * g / groups);
+    const int h1 = static_cast<int>(static_cast<long long>(H) * (g + 1) / groups);
+    const size_t n = sa_fwd_workspace_bytes(1, h1 - h0, N, Bq);
+    need = n > need ? n : need;
+  }
+  return need;
+}
+
 size_t sa_fwd_host_scratch_bytes(int B, int H, int N, int D, int Bq, int Bk) {
   if (B <= 0 || H <= 0 || N <= 0 || D <= 0 || Bq <= 0 || Bk <= 0 || N % Bq || N % Bk) return 0;
   const size_t t = al256(static_cast<size_t>(B) * H * N * D * 2);
   const size_t l = al256(static_cast<size_t>(B) * H * N * 4);
   const size_t m = al256(static_cast<size_t>(H) * (N / Bq) * ((N / Bk + 31) / 32) * 4);
-  return 4 * t + l + m + sa_fwd_workspace_bytes(B, H, N, Bq);
+  return 4 * t + l + m + host_pipeline_ws_bytes(H, N, Bq);
 }
 
 sa_status sa_pack_mask(const float* scores, const float* density, uint32_t* mask_bits, int H,
@@ -476,7 +491,7 @@ static sa_status pipelined_fwd_host(const void* q_host, const void* k_host, cons
     return cuda_fail(e, "copy pipeline fork");
   const size_t row_bytes = static_cast<size_t>(N) * D * 2;
   const size_t mask_head_bytes = static_cast<size_t>(N / Bq) * ((N / Bk + 31) / 32) * 4;
-  const size_t ws_bytes = sa_fwd_workspace_bytes(B, H, N, Bq);
+  const size_t ws_bytes = host_pipeline_ws_bytes(H, N, Bq);
   int c = 0;
   for (int b = 0; b < B; ++b) {
     for (int g = 0; g < groups; ++g, ++c) {
@@ -573,7 +588,7 @@ sa_status sa_hot_path_host(const float* scores_host, const float* density_host, 
   const size_t lb = static_cast<size_t>(B) * H * N * 4, l = al256(lb);
   const size_t mb = static_cast<size_t>(H) * NQB * ((NKB + 31) / 32) * 4, m = al256(mb);
   const size_t sb = static_cast<size_t>(H) * NQB * NKB * 4, db = static_cast<size_t>(H) * 4;
-  const size_t fwd_ws = sa_fwd_workspace_bytes(B, H, N, Bq);
+  const size_t fwd_ws = host_pipeline_ws_bytes(H, N, Bq);
   const size_t pack_ws = sa_pack_mask_workspace_bytes(H, NQB, NKB);
   char* base = static_cast<char*>(scratch);
   char *dq = base, *dk = base + t, *dv = base + 2 * t, *dout = base + 3 * t;

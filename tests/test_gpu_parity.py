@@ -899,6 +899,45 @@ def test_host_entry_points_pipelined_head_groups(sa):
     check_out(out, lse, ref_o, ref_l, "sa_block_sparse_attn_fwd_host")
 
 
+def test_host_entry_point_head_groups_with_parts(sa):
+    # H = 64 at N = 9600: the whole problem (2432 pairs) keeps whole rows, but each of the 8 head groups
+    # the host form runs (304 pairs on 148 SMs) issues its last round in parts: the shared workspace
+    # must be sized for the groups, and the result equals the device call on each head group, bit for bit.
+    D, blk, H, N = 128, 128, 64, 9600
+    g = torch.Generator().manual_seed(61)
+    q, k, v = [torch.randn((1, H, N, D), generator=g).to(torch.bfloat16).pin_memory() for _ in range(3)]
+    rng = np.random.Generator(np.random.PCG64(62))
+    m = rng.random((H, N // blk, N // blk)) < 0.9
+    bits = oracle.pack_bool(m)
+    scale = float(np.float32(1 / math.sqrt(D)))
+    out = torch.empty_like(q).pin_memory()
+    lse = torch.empty((1, H, N), dtype=torch.float32).pin_memory()
+    bits_h = torch.from_numpy(bits.view(np.int32)).pin_memory()
+    scratch = torch.empty(sa.sa_fwd_host_scratch_bytes(1, H, N, D, blk, blk), dtype=torch.uint8, device="cuda")
+    sa.sa_block_sparse_attn_fwd_host(q, k, v, bits_h, out, lse, blk, blk, scale, N, scratch)
+    torch.cuda.synchronize()
+    qd, kd, vd = q.cuda(), k.cuda(), v.cuda()
+    launches = set()
+    for g8 in range(8):
+        h0, h1 = H * g8 // 8, H * (g8 + 1) // 8
+        o, l = sa.sa_block_sparse_attn_fwd_ex(qd[:, h0:h1].contiguous(), kd[:, h0:h1].contiguous(),
+                                              vd[:, h0:h1].contiguous(), dev_bits(bits[h0:h1]), blk, blk, scale)
+        launches.add(sa.sa_last_launch_count())
+        torch.cuda.synchronize()
+        assert torch.equal(o.cpu(), out[:, h0:h1]) and torch.equal(l.cpu(), lse[:, h0:h1])
+    assert launches == {4}                                    # every group ran its last round in parts
+    # the mask-pack + attention form, its scratch carved behind the same workspace
+    scores, density = inputs.bool_mask_as_scores(m)
+    out2 = torch.empty_like(q).pin_memory()
+    lse2 = torch.empty_like(lse).pin_memory()
+    bits2 = torch.zeros_like(bits_h).pin_memory()
+    scratch2 = torch.empty(sa.sa_hot_path_host_scratch_bytes(1, H, N, D, blk, blk), dtype=torch.uint8, device="cuda")
+    sa.sa_hot_path_host(torch.from_numpy(scores).pin_memory(), torch.from_numpy(density).pin_memory(),
+                        q, k, v, bits2, out2, lse2, blk, blk, scale, N, scratch2, force_diag=False)
+    torch.cuda.synchronize()
+    assert torch.equal(bits2, bits_h) and torch.equal(out2, out) and torch.equal(lse2, lse)
+
+
 @pytest.mark.parametrize("D,blk", [(128, 128), (64, 64)])
 def test_schedule_reuse_is_bit_identical(sa, D, blk):
     # the static-mask form: the work list of an earlier call is reused ("Reuse for All
