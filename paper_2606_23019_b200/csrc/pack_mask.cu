@@ -171,6 +171,7 @@ pack_hist_kernel(const float* __restrict__ scores, const float* __restrict__ den
   constexpr int nb = 1 << digit_bits(PASS);
   constexpr int shift = digit_shift(PASS);
   const int h = blockIdx.y;
+  if (PASS > 0) griddep_wait();       // (launched programmatically behind the previous pass)
   resolve(PASS, h, density, NQB, NKB, force_diag, hist, state, s_hist, &s_prefix, &s_krem,
           blockIdx.x == 0);
   const uint32_t prefix = s_prefix;
@@ -237,6 +238,7 @@ pack_row_ties_kernel(const float* __restrict__ scores, const float* __restrict__
   __shared__ uint32_t s_bins[kBins];
   __shared__ uint32_t s_T, s_r, s_neq;
   const int h = blockIdx.y;
+  griddep_wait();
   resolve(kPasses, h, density, NQB, NKB, force_diag, hist, state, s_bins, &s_T, &s_r,
           blockIdx.x == 0, &s_neq);
   const uint32_t T = s_T;
@@ -266,6 +268,7 @@ pack_write_kernel(const float* __restrict__ scores, int NQB, int NKB, int W, int
   const int h = blockIdx.y;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int u = blockIdx.x * 8 + warp;
+  griddep_wait();
   if (u >= NQB) return;
   const uint32_t T = state[h].prefix[kPasses];
   const uint32_t r = state[h].k_rem[kPasses];
@@ -361,12 +364,25 @@ cudaError_t launch_pack_mask(const float* scores, const float* density, uint32_t
   chunk = (chunk + 1023) / 1024 * 1024;
   dim3 hgrid(static_cast<unsigned>((total + chunk - 1) / chunk), H);
   pack_hist_kernel<0><<<hgrid, kHistThreads, 0, st>>>(scores, density, NQB, NKB, force_diag, chunk, w.hist, w.state);
-  pack_hist_kernel<1><<<hgrid, kHistThreads, 0, st>>>(scores, density, NQB, NKB, force_diag, chunk, w.hist, w.state);
-  pack_hist_kernel<2><<<hgrid, kHistThreads, 0, st>>>(scores, density, NQB, NKB, force_diag, chunk, w.hist, w.state);
+  // the dependent kernels are launched programmatically: their launch overlaps the previous pass
+  uint32_t* hist = w.hist;
+  HeadState* state = w.state;
+  const HeadState* cstate = w.state;
+  const uint32_t* chist = w.hist;
+  const uint32_t* cties = w.row_ties;
+  if ((e = launch_pdl(pack_hist_kernel<1>, hgrid, dim3(kHistThreads), 0, st, scores, density, NQB, NKB, force_diag,
+                      chunk, hist, state)) != cudaSuccess ||
+      (e = launch_pdl(pack_hist_kernel<2>, hgrid, dim3(kHistThreads), 0, st, scores, density, NQB, NKB, force_diag,
+                      chunk, hist, state)) != cudaSuccess)
+    return e;
   dim3 tgrid((NQB + kTieRowsPerBlock - 1) / kTieRowsPerBlock, H);
-  pack_row_ties_kernel<<<tgrid, 256, 0, st>>>(scores, density, NQB, NKB, force_diag, w.hist, w.state, w.row_ties);
+  if ((e = launch_pdl(pack_row_ties_kernel, tgrid, dim3(256), 0, st, scores, density, NQB, NKB, force_diag, chist,
+                      state, w.row_ties)) != cudaSuccess)
+    return e;
   dim3 rgrid((NQB + 7) / 8, H);
-  pack_write_kernel<<<rgrid, 256, 0, st>>>(scores, NQB, NKB, W, force_diag, w.state, w.row_ties, mask_bits);
+  if ((e = launch_pdl(pack_write_kernel, rgrid, dim3(256), 0, st, scores, NQB, NKB, W, force_diag, cstate, cties,
+                      mask_bits)) != cudaSuccess)
+    return e;
   return cudaGetLastError();
 }
 

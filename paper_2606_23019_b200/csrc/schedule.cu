@@ -194,6 +194,7 @@ schedule_items_kernel(const uint32_t* __restrict__ mask_bits, int H, int NQB, in
   }
   for (int i = threadIdx.x; i < n2; i += blockDim.x) s_keys[i] = 0u;
   for (int i = threadIdx.x; i < slots; i += blockDim.x) s_a[i] = s_b[i] = 0xFFFFu;
+  griddep_wait();        // (launched programmatically: the mask may come from the kernel just before)
   __syncthreads();
 
   // ---- popcount of every row (one warp per row, lanes over the words)
@@ -656,10 +657,10 @@ cudaError_t launch_schedule(const FwdParams& p, const FwdWorkspace& w, int rpi, 
                               200 * 1024);
       if (e != cudaSuccess) return e;
     }
-    schedule_items_kernel<<<BH, kSortThreads, smem, st>>>(p.mask_bits, p.H, p.NQB, p.NKB, p.W, rpi == 2 ? 1 : 0,
-                                                         p.split_rows, rpi == 2 ? plan.rem : 0, plan.parts, n2,
-                                                         w.head_cost, w.head_count, w.head_tail, w.local_items,
-                                                         w.tasks, w.part_mask, w.kmax2);
+    e = launch_pdl(schedule_items_kernel, dim3(BH), dim3(kSortThreads), smem, st, p.mask_bits, p.H, p.NQB, p.NKB,
+                   p.W, rpi == 2 ? 1 : 0, p.split_rows, rpi == 2 ? plan.rem : 0, plan.parts, n2, w.head_cost,
+                   w.head_count, w.head_tail, w.local_items, w.tasks, w.part_mask, w.kmax2);
+    if (e != cudaSuccess) return e;
     *n_launch += 1;
   }
   if (!reuse || norms) {
