@@ -272,6 +272,12 @@ SA_API sa_status sa_debug_fwd_walk(const void* q, const void* k, const void* v, 
                                    int Bk, float scale, void* workspace, size_t workspace_bytes,
                                    int32_t* walk_log, size_t walk_log_bytes, void* stream);
 
+/* Debug hook (host arithmetic only, no CUDA call): the plan a forward call of this shape follows for the
+ * partly filled last round of its pair items on a device with n_sm SMs (K2): *rem work
+ * items (spread over the B*H groups, each group's lightest) are issued in *parts parts over key ranges
+ * and merged afterwards; 0 / 0 when every item stays whole. SA_ERR_INVALID_ARG on bad sizes. */
+SA_API sa_status sa_debug_tail_plan(int B, int H, int N, int Bq, int Bk, int n_sm, int* rem, int* parts);
+
 /* Number of kernels the last sa_pack_mask / forward / sa_hot_path_host call on this thread
  * enqueued (for bench accounting; memsets and copies are not counted). */
 SA_API int sa_last_launch_count(void);

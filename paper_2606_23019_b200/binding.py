@@ -70,6 +70,8 @@ def load_library() -> C.CDLL:
     lib.sa_block_sparse_attn_fwd_reuse.argtypes = lib.sa_block_sparse_attn_fwd_ex.argtypes
     lib.sa_fwd_softmax_path_counts.restype = ip
     lib.sa_fwd_softmax_path_counts.argtypes = [vp, vp, vp, vp]
+    lib.sa_debug_tail_plan.restype = ip
+    lib.sa_debug_tail_plan.argtypes = [ip, ip, ip, ip, ip, ip, vp, vp]
     lib.sa_debug_ex2_rate.restype = ip
     lib.sa_debug_ex2_rate.argtypes = [ip, vp, vp, vp, vp]
     lib.sa_debug_fwd_walk_log_bytes.restype = sz
@@ -309,6 +311,14 @@ def sa_fwd_softmax_path_counts(workspace, stream=None):
     _check(load_library().sa_fwd_softmax_path_counts(_ptr(workspace), C.addressof(a), C.addressof(b),
                                                      _stream(stream)))
     return a.value, b.value
+
+
+def sa_debug_tail_plan(B: int, H: int, N: int, Bq: int, Bk: int, n_sm: int):
+    """(rem, parts): how many work items a forward call of this shape issues in how many parts each
+    on a device with n_sm SMs (host arithmetic only)."""
+    rem, parts = C.c_int(0), C.c_int(0)
+    _check(load_library().sa_debug_tail_plan(B, H, N, Bq, Bk, n_sm, C.addressof(rem), C.addressof(parts)))
+    return rem.value, parts.value
 
 
 def sa_debug_ex2_rate(seconds: float = 0.5, iters: int = 4096, device=None, stream=None):

@@ -406,6 +406,15 @@ sa_status sa_block_sparse_attn_fwd_ex(const void* q, const void* k, const void* 
                      workspace_bytes, stream, false);
 }
 
+sa_status sa_debug_tail_plan(int B, int H, int N, int Bq, int Bk, int n_sm, int* rem, int* parts) {
+  if (!rem || !parts || B <= 0 || H <= 0 || N <= 0 || Bq <= 0 || Bk <= 0 || N % Bq || N % Bk || n_sm <= 0)
+    return fail(SA_ERR_INVALID_ARG, "sa_debug_tail_plan: bad sizes or null pointer");
+  const sa::TailPlan t = sa::fwd_tail_plan(B, H, N / Bq, N / Bk, n_sm);
+  *rem = t.rem;
+  *parts = t.parts;
+  return SA_OK;
+}
+
 size_t sa_debug_fwd_walk_log_bytes(int B, int H, int N, int Bq, int Bk) {
   if (B <= 0 || H <= 0 || N <= 0 || Bq <= 0 || Bk <= 0 || N % Bq || N % Bk) return 0;
   const size_t rows = static_cast<size_t>(B) * H * (N / Bq), nkb = static_cast<size_t>(N / Bk);

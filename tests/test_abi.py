@@ -51,6 +51,27 @@ def test_host_helpers(lib):
     assert lib.sa_status_string(2) == b"SA_ERR_UNSUPPORTED"
 
 
+def test_tail_plan_host_logic():
+    # DESIGN.md K2: P pair items on n SMs; rem = P mod n items run in `parts` parts when that makes the
+    # last round ceil(rem * parts / n) / parts of a pair long, saves >= 3% of the launch, and a dense row
+    # has 32 key blocks per part. Worked by hand:
+    from paper_2606_23019_b200 import binding as sa
+    plan = lambda H, N, n=148, B=1: sa.sa_debug_tail_plan(B, H, N, 128, 128, n)
+    assert plan(12, 16384) == (28, 4)        # 768 pairs = 5 x 148 + 28; 112 quarter items fill 3/4 of a round
+    assert plan(12, 32768) == (56, 2)        # 1536 = 10 x 148 + 56; halves and quarters both give 1/2: fewer parts
+    assert plan(12, 8192) == (0, 0)          # 384 = 2 x 148 + 88, 64 key blocks: halves only, 176 halves = a whole round
+    assert plan(12, 65536) == (0, 0)         # 3072 = 20 x 148 + 112: no split shortens the round
+    assert plan(40, 75648) == (0, 0)         # C4: 11840 pairs = 80 rounds exactly
+    assert plan(24, 44672) == (0, 0)         # HunyuanVideo shape: 4200 = 28 x 148 + 56: half a round of 29 is < 3%
+    assert plan(12, 4096) == (0, 0)          # below two waves of pairs: split items instead (api.cu)
+    assert plan(8, 9600) == (8, 2)           # 304 pairs; 75 key blocks allow two parts
+    assert plan(5, 16384) == (24, 4)
+    # 29 rounds + 1 item: one quarter of a round saved is < 3% of 30 rounds
+    assert plan(1, 128 * 2 * (148 * 29 + 1)) == (0, 0)
+    with pytest.raises(sa.SAError):
+        sa.sa_debug_tail_plan(1, 12, 1000, 128, 128, 148)
+
+
 def _fwd_ex(lib, q=16, k=16, v=16, m=16, o=16, l=16, B=1, H=2, N=1024, nv=1024, D=64, Bq=64,
             Bk=64, scale=0.125, ws=16, wsb=1 << 20):
     return lib.sa_block_sparse_attn_fwd_ex(q, k, v, m, o, l, B, H, N, nv, D, Bq, Bk, scale, ws,
