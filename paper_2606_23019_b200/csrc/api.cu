@@ -121,6 +121,20 @@ std::mutex g_pipe_mu;
 constexpr int kMaxPipeDevices = 64;
 PipeCtx g_pipes[kMaxPipeDevices];   // streams and events belong to a device: one context per ordinal
 constexpr int kPipeGroups = 8;     // head groups per batch entry (fewer when H is small)
+// First head of group g (g = groups: H). The groups taper towards the end -- weights 3 3 3 3 3 3 2 1 -- so
+// that what cannot overlap anything, the last group's compute and download, is short.
+static int pipe_group_begin(int H, int groups, int g) {
+  if (groups < kPipeGroups) return static_cast<int>(static_cast<long long>(H) * g / groups);   // one head each
+  static const int cum[kPipeGroups + 1] = {0, 3, 6, 9, 12, 15, 18, 20, 21};
+  int prev = 0;
+  for (int i = 1; i <= g; ++i) {
+    int h = static_cast<int>((static_cast<long long>(H) * cum[i] * 2 + 21) / 42);   // round(H cum / 21)
+    h = h < prev + 1 ? prev + 1 : h;                                                 // every group has a head
+    const int room = H - (groups - i);                                               // and leaves one for each later group
+    prev = h > room ? room : h;
+  }
+  return prev;
+}
 
 }  // namespace
 
@@ -161,8 +175,7 @@ static size_t host_pipeline_ws_bytes(int H, int N, int Bq) {
   const int groups = H < kPipeGroups ? H : kPipeGroups;
   size_t need = 0;
   for (int g = 0; g < groups; ++g) {
-    const int h0 = static_cast<int>(static_cast<long long>(H) * g / groups);
-    const int h1 = static_cast<int>(static_cast<long long>(H) * (g + 1) / groups);
+    const int h0 = pipe_group_begin(H, groups, g), h1 = pipe_group_begin(H, groups, g + 1);
     const size_t n = sa_fwd_workspace_bytes(1, h1 - h0, N, Bq);
     need = n > need ? n : need;
   }
@@ -504,8 +517,7 @@ static sa_status pipelined_fwd_host(const void* q_host, const void* k_host, cons
   int c = 0;
   for (int b = 0; b < B; ++b) {
     for (int g = 0; g < groups; ++g, ++c) {
-      const int h0 = static_cast<int>(static_cast<long long>(H) * g / groups);
-      const int h1 = static_cast<int>(static_cast<long long>(H) * (g + 1) / groups);
+      const int h0 = pipe_group_begin(H, groups, g), h1 = pipe_group_begin(H, groups, g + 1);
       const size_t off = (static_cast<size_t>(b) * H + h0) * row_bytes;
       const size_t bytes = static_cast<size_t>(h1 - h0) * row_bytes;
       const size_t loff = (static_cast<size_t>(b) * H + h0) * N * 4, lbytes = static_cast<size_t>(h1 - h0) * N * 4;
