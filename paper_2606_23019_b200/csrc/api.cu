@@ -377,6 +377,9 @@ static sa_status fwd_ex_impl(const void* q, const void* k, const void* v, const 
   // the partly filled last round of pair items is issued in parts over key ranges (schedule.cu)
   const sa::TailPlan plan = (fast && variant == 0 && rows_per_item == 2 && p.NKB <= 0xFFFF)
                                 ? sa::fwd_tail_plan(B, H, p.NQB, p.NKB, n_sm) : sa::TailPlan{};
+  // large problems without parts run the lean build of the kernel (no split items, no parts: the
+  // one leftover row of an odd head becomes a single-row item there, which at >= 8 rounds is noise)
+  p.lean_items = (fast && variant == 0 && rows_per_item == 2 && plan.parts == 0 && n_pairs >= 8LL * n_sm) ? 1 : 0;
   p.part_mask = w.part_mask;
   p.part_out = w.part_out;
   p.part_lse = w.part_lse;

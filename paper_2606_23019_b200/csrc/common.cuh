@@ -71,6 +71,7 @@ struct FwdParams {
   int n_items;                // host-side count: exact for single-row items, an upper bound for pairs
   int rows_per_item;          // query blocks per work item: 2 (a pair shares its K/V tiles) or 1
   int split_rows;             // single-row items are split items (tcgen05 kernel): see Item::split
+  int lean_items;             // the work list holds no split item and no part: the lean kernel build runs it
   int32_t* stats;             // [2] (warp, item) counts by softmax path: fixed reference point / exact
                               // running max (zeroed by the pre-pass; tcgen05 kernel only)
   int32_t* walk_log;          // sa_debug_fwd_walk only (else null): see WalkLog in fwd_tcgen05.cu
@@ -115,7 +116,7 @@ FwdWorkspace carve_fwd_workspace(void* ws, int B, int H, int NQB, int W, TailPla
 
 // per-device state (device.cu): SM count of the current device; dynamic shared-memory opt-in of a
 // kernel, set once per (device, kernel)
-enum SmemKernel { kSmemFwdTcgen05 = 0, kSmemFwdTcgen05Log, kSmemSigTcgen05, kSmemScheduleItems, kSmemFwdMmaSync64,
+enum SmemKernel { kSmemFwdTcgen05 = 0, kSmemFwdTcgen05Lean, kSmemFwdTcgen05Log, kSmemSigTcgen05, kSmemScheduleItems, kSmemFwdMmaSync64,
                   kSmemFwdMmaSync128, kSmemMaskFromThreshold, kNumSmemKernels };
 cudaError_t device_sm_count(int* n_sm);
 cudaError_t ensure_dynamic_smem(SmemKernel id, const void* func, int bytes);

@@ -111,7 +111,10 @@ constexpr uint32_t kIdescPV = kIdescQK | (1u << 16);
 
 // A work item: query blocks ua (tile 0) and ub (tile 1) of one (batch, head); the schedule pre-pass
 // chooses the pairs (schedule.cu). Single-row items leave tile 1 empty.
-struct Item {
+// (kFull = false: the LEAN build of the kernel, for launches whose work list holds neither split items nor
+// parts -- large problems: the code of both is compiled out, which is worth ~1.5% at C4.)
+template <bool kFull>
+struct ItemT {
   int bh, h, ua, ub;
   bool has1;
   int row0;            // first token row of the (b,h) slab in the [B*H*N][D] view
@@ -120,19 +123,20 @@ struct Item {
   // ub == ua: a SPLIT item -- ONE query block whose key blocks are dealt to the two tiles in turn (even
   // key blocks -> tile 0, odd -> tile 1), the halves merged in the epilogue. (Derived on demand: the
   // softmax loop has no register to spare for another live flag.)
-  __device__ __forceinline__ bool split() const { return ub == ua; }
+  __device__ __forceinline__ bool split() const { return kFull && ub == ua; }
 };
 // item record: x = b*H + h (-1: no more work), y = ua | ub << 16 (ub = 0xFFFF: no second row),
 // z = scratch slot of a part (-1: the item covers its rows' whole bit-rows and writes out / lse itself)
-__device__ __forceinline__ Item decode_item(const FwdParams& p, int4 rec) {
-  Item it;
+template <bool kFull>
+__device__ __forceinline__ ItemT<kFull> decode_item(const FwdParams& p, int4 rec) {
+  ItemT<kFull> it;
   it.bh = rec.x;
   it.h = it.bh % p.H;
   it.ua = rec.y & 0xFFFF;
   it.ub = (rec.y >> 16) & 0xFFFF;
   it.has1 = it.ub != 0xFFFF;
   it.row0 = it.bh * p.N;
-  it.part = rec.z;
+  it.part = kFull ? rec.z : -1;
   return it;
 }
 
@@ -173,6 +177,7 @@ __device__ __forceinline__ uint32_t row_word(const FwdParams& p, int h, int u, i
 // the result is too.
 struct RowWalk {
   uint32_t a0 = 0, a1 = 0, b0 = 0, b1 = 0;
+  template <class Item>
   __device__ __forceinline__ void load(const FwdParams& p, const Item& it, int base, int lane) {
     const int w0 = base + lane, w1 = base + 32 + lane;
     a0 = w0 < p.W ? row_word(p, it.h, it.ua, w0, true, it.part, 0) : 0u;
@@ -210,6 +215,7 @@ struct Ring {
 
 // ------------------------------------------------------------------ warp 0: scheduler + TMA
 // Runs on every lane of warp 0 (converged); elect.sync inside the _e wrappers picks the issuer.
+template <bool kFull>
 __device__ void producer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, const CUtensorMap* tm_q,
                          const CUtensorMap* tm_k, const CUtensorMap* tm_v, int lane) {
   Ring ring;
@@ -240,7 +246,7 @@ __device__ void producer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, const
   for (;;) {
     const int4 item = next_item;
     if (item.x < 0) break;
-    const Item it = decode_item(p, item);
+    const ItemT<kFull> it = decode_item<kFull>(p, item);
     // ... unless this item is a long one (a held-back item would then wait that long while another
     // CTA may be idle): long items claim their successor only when their own loads are out
     RowWalk rw;
@@ -317,7 +323,7 @@ struct Pend {
 // tiles has still ping-pongs between the two S buffers. Issue order: PV(w-2), S(w): the softmax of
 // unit w-1 overlaps both. P(w-2) aliases S buffer (w & 1), so S(w) must follow PV(w-2) in the
 // (in-order) tensor pipe, which this order guarantees.
-template <bool kLog>
+template <bool kLog, bool kFull>
 __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uint32_t tmem,
                            int lane) {
   Ring ring;
@@ -371,7 +377,7 @@ __device__ void mma_issuer(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     if (lane == 0) mbar_arrive(smem_u32(&ctl->sched_empty[ss]));
     ++sched_n;
     if (item.x < 0) break;
-    const Item it = decode_item(p, item);
+    const ItemT<kFull> it = decode_item<kFull>(p, item);
 
     RowWalk rw;
     uint32_t rem[2] = {0, 0};            // units each tile still has in this item
@@ -561,7 +567,7 @@ __device__ __forceinline__ float exp_tile(const uint32_t (&sr)[4][32], float c, 
 // ------------------------------------------------------------------ warps 4-11: softmax + epilogue
 // One thread per query row: thread (quarter, lane) of warpgroup t owns TMEM lane 32*quarter+lane
 // of S_t / O_t, so row max and row sum need no shuffles.
-template <bool kLog>
+template <bool kLog, bool kFull>
 __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uint32_t tmem, int t,
                            int quarter, int lane) {
   const int row = quarter * 32 + lane;
@@ -581,7 +587,7 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
   // the next item from the scheduler ring and waits for its Q tiles; it is called for item n+1
   // BEFORE the epilogue of item n, so that the wait for the Q tiles and the row norms fall into the
   // time this warpgroup would otherwise spend waiting for the last PV of item n.
-  Item it{};
+  ItemT<kFull> it{};
   bool exists = false;
   RowWalk rw;
   float bound = 0.f;
@@ -595,7 +601,7 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     if (lane == 0) mbar_arrive(smem_u32(&ctl->sched_empty[ss]));
     ++sched_n;
     if (item.x < 0) return false;
-    it = decode_item(p, item);
+    it = decode_item<kFull>(p, item);
     exists = t == 0 || it.has1;   // tile 1 is empty in single-row items and past the last row
 
     // An upper bound of every score of this query row (Cauchy-Schwarz): scale * |q_i| * max_j |k_j|,
@@ -893,7 +899,7 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
 }
 
 // ------------------------------------------------------------------ kernel
-template <bool kLog>
+template <bool kLog, bool kFull>
 __global__ void __launch_bounds__(kThreads, 1)
 fwd_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
                    const __grid_constant__ CUtensorMap tm_v, const FwdParams p) {
@@ -947,13 +953,13 @@ fwd_tcgen05_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_consta
   if (warp < 4) {
     setmaxnreg_dec<88>();
     if (warp == 0) {
-      producer(p, ctl, smem_base, &tm_q, &tm_k, &tm_v, lane);
+      producer<kFull>(p, ctl, smem_base, &tm_q, &tm_k, &tm_v, lane);
     } else if (warp == 1) {
-      mma_issuer<kLog>(p, ctl, smem_base, tmem, lane);
+      mma_issuer<kLog, kFull>(p, ctl, smem_base, tmem, lane);
     }
   } else {
     setmaxnreg_inc<208>();
-    softmax_wg<kLog>(p, ctl, smem_base, tmem, warp >= 8 ? 1 : 0, warp & 3, lane);
+    softmax_wg<kLog, kFull>(p, ctl, smem_base, tmem, warp >= 8 ? 1 : 0, warp & 3, lane);
   }
   tc_fence_before();
   __syncthreads();
@@ -1004,10 +1010,14 @@ cudaError_t launch_fwd_tcgen05(const FwdParams& p, void*, cudaStream_t st, int* 
   cudaError_t e = device_sm_count(&n_sm);
   if (e != cudaSuccess) return e;
   const bool log = p.walk_log != nullptr;
-  e = log ? ensure_dynamic_smem(kSmemFwdTcgen05Log, reinterpret_cast<const void*>(fwd_tcgen05_kernel<true>),
+  const bool lean = !log && p.lean_items;        // the work list holds neither split items nor parts
+  e = log ? ensure_dynamic_smem(kSmemFwdTcgen05Log, reinterpret_cast<const void*>(fwd_tcgen05_kernel<true, true>),
                                 static_cast<int>(kSmemBytes))
-          : ensure_dynamic_smem(kSmemFwdTcgen05, reinterpret_cast<const void*>(fwd_tcgen05_kernel<false>),
-                                static_cast<int>(kSmemBytes));
+          : lean ? ensure_dynamic_smem(kSmemFwdTcgen05Lean,
+                                       reinterpret_cast<const void*>(fwd_tcgen05_kernel<false, false>),
+                                       static_cast<int>(kSmemBytes))
+                 : ensure_dynamic_smem(kSmemFwdTcgen05, reinterpret_cast<const void*>(fwd_tcgen05_kernel<false, true>),
+                                       static_cast<int>(kSmemBytes));
   if (e != cudaSuccess) { *err_text = "cudaFuncSetAttribute(fwd_tcgen05_kernel)"; return e; }
   CUtensorMap tq, tk, tv;
   const uint64_t rows = static_cast<uint64_t>(p.B) * p.H * p.N;
@@ -1016,8 +1026,11 @@ cudaError_t launch_fwd_tcgen05(const FwdParams& p, void*, cudaStream_t st, int* 
     return cudaErrorInvalidValue;
   }
   const int grid = p.n_items < n_sm ? p.n_items : n_sm;   // n_items: upper bound (pairs are mask-dependent)
-  e = log ? launch_pdl(fwd_tcgen05_kernel<true>, dim3(grid), dim3(kThreads), kSmemBytes, st, tq, tk, tv, p)
-          : launch_pdl(fwd_tcgen05_kernel<false>, dim3(grid), dim3(kThreads), kSmemBytes, st, tq, tk, tv, p);
+  e = log ? launch_pdl(fwd_tcgen05_kernel<true, true>, dim3(grid), dim3(kThreads), kSmemBytes, st, tq, tk, tv, p)
+          : lean ? launch_pdl(fwd_tcgen05_kernel<false, false>, dim3(grid), dim3(kThreads), kSmemBytes, st, tq, tk,
+                              tv, p)
+                 : launch_pdl(fwd_tcgen05_kernel<false, true>, dim3(grid), dim3(kThreads), kSmemBytes, st, tq, tk,
+                              tv, p);
   if (e != cudaSuccess) return e;
   *n_launch += 1;
   return cudaGetLastError();

@@ -169,7 +169,7 @@ __device__ __forceinline__ int pow2_at_least(int n) {
 // Dynamic shared memory: keys[n2] (uint32), then pop[NQB], ia[slots], ib[slots] (uint16).
 __global__ void __launch_bounds__(kSortThreads)
 schedule_items_kernel(const uint32_t* __restrict__ mask_bits, int H, int NQB, int NKB, int W,
-                      int pair_rows, int split_rows, int plan_rem, int plan_parts, int n2,
+                      int pair_rows, int split_rows, int split_leftover, int plan_rem, int plan_parts, int n2,
                       int32_t* __restrict__ head_cost, int32_t* __restrict__ head_count,
                       int32_t* __restrict__ head_tail, int4* __restrict__ local_items,
                       int4* __restrict__ tasks, uint32_t* __restrict__ part_mask,
@@ -281,13 +281,14 @@ schedule_items_kernel(const uint32_t* __restrict__ mask_bits, int H, int NQB, in
         }
         if (lane == 0) {
           // a row left without a partner becomes a split item (ub = ua): its key blocks alternate
-          // between the kernel's two tiles, so that both softmax warpgroups work on it
+          // between the kernel's two tiles, so that both softmax warpgroups work on it (a single-row
+          // item, ub = 0xFFFF, when the launch runs the lean kernel build, which has no split items)
           const int s = n_adj + 2 * g;
           s_a[s] = static_cast<uint16_t>(r[0]);
-          s_b[s] = static_cast<uint16_t>(r[p0] >= 0 ? r[p0] : r[0]);
+          s_b[s] = static_cast<uint16_t>(r[p0] >= 0 ? r[p0] : (split_leftover ? r[0] : 0xFFFF));
           if (r[p1] >= 0) {
             s_a[s + 1] = static_cast<uint16_t>(r[p1]);
-            s_b[s + 1] = static_cast<uint16_t>(r[p2] >= 0 ? r[p2] : r[p1]);
+            s_b[s + 1] = static_cast<uint16_t>(r[p2] >= 0 ? r[p2] : (split_leftover ? r[p1] : 0xFFFF));
           }
         }
       }
@@ -658,7 +659,8 @@ cudaError_t launch_schedule(const FwdParams& p, const FwdWorkspace& w, int rpi, 
       if (e != cudaSuccess) return e;
     }
     e = launch_pdl(schedule_items_kernel, dim3(BH), dim3(kSortThreads), smem, st, p.mask_bits, p.H, p.NQB, p.NKB,
-                   p.W, rpi == 2 ? 1 : 0, p.split_rows, rpi == 2 ? plan.rem : 0, plan.parts, n2, w.head_cost,
+                   p.W, rpi == 2 ? 1 : 0, p.split_rows, p.lean_items ? 0 : 1, rpi == 2 ? plan.rem : 0, plan.parts, n2,
+                   w.head_cost,
                    w.head_count, w.head_tail, w.local_items, w.tasks, w.part_mask, w.kmax2);
     if (e != cudaSuccess) return e;
     *n_launch += 1;
