@@ -37,7 +37,7 @@ UNIT = "TFLOP/s"
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the attention kernel at the bench
 # workload, from the `ncu --set full` capture summarised in profiles/ (None until captured).
-NCU_TRAFFIC_BYTES = {"C4": 3342828760}   # dram__bytes_read.sum + dram__bytes_write.sum, one launch
+NCU_TRAFFIC_BYTES = {"C4": 3335543864}   # dram__bytes_read.sum + dram__bytes_write.sum, one launch
 NCU_TRAFFIC_SOURCE = {"C4": "profiles/r2_fwd_tcgen05_c4_full.md"}
 
 
