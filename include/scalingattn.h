@@ -72,6 +72,22 @@ SA_API sa_status sa_pack_mask(const float* scores, const float* density, uint32_
                        int NQB, int NKB, int force_diag, void* workspace, size_t workspace_bytes,
                        void* stream);
 
+/* sa_pack_mask for callers that cannot allocate device memory (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc): same operation, same arguments and results, but
+ * the workspace is a fixed array inside the library, SA_STATIC_SCRATCH_BYTES (2.25 MiB) of device
+ * memory that every GPU which loads the library holds until the process exits. The call allocates
+ * and frees nothing (no cudaMalloc / cudaFree, no allocating library routine); the first call on a
+ * device looks the array's address up (cudaGetSymbolAddress), later calls reuse it.
+ * Limit: sa_pack_mask_workspace_bytes(H, NQB, NKB) <= SA_STATIC_SCRATCH_BYTES, e.g. H <= 64 heads at
+ * up to 2048 x 2048 blocks; SA_ERR_WORKSPACE beyond it (the message names both sizes).
+ * All calls on a device share the array: calls ordered on one stream (or by events) are safe, calls
+ * that overlap on the GPU race on it and give undefined masks. Nothing is carried from call to call
+ * (the histograms are zeroed on `stream` at the start of every call). Bit-exact and deterministic
+ * like sa_pack_mask; 5 kernels and one memset on `stream`, no synchronisation. */
+#define SA_STATIC_SCRATCH_BYTES (2304 * 1024)
+SA_API sa_status sa_pack_mask_static(const float* scores, const float* density, uint32_t* mask_bits,
+                                     int H, int NQB, int NKB, int force_diag, void* stream);
+
 /* The paper's run-time mask path: a per-head THRESHOLD MAP kept at a base resolution, instantiated
  * at the target resolution (PAPER.md:103 M_p = 1(T <= p); Eq. 7, the conservative
  * bilinear resize with a ceiling rule; readings P14-P16):

@@ -51,6 +51,8 @@ def load_library() -> C.CDLL:
     lib.sa_fwd_host_scratch_bytes.argtypes = [ip] * 6
     lib.sa_pack_mask.restype = ip
     lib.sa_pack_mask.argtypes = [vp, vp, vp, ip, ip, ip, ip, vp, sz, vp]
+    lib.sa_pack_mask_static.restype = ip
+    lib.sa_pack_mask_static.argtypes = [vp, vp, vp, ip, ip, ip, ip, vp]
     lib.sa_mask_from_threshold.restype = ip
     lib.sa_mask_from_threshold.argtypes = [vp, vp, vp, ip, ip, ip, ip, ip, ip, vp]
     lib.sa_block_significance.restype = ip
@@ -185,6 +187,24 @@ def sa_pack_mask(scores, density, force_diag: bool = True, mask_bits=None, works
     _check(lib.sa_pack_mask(_ptr(scores), _ptr(density), _ptr(mask_bits), H, NQB, NKB,
                             int(bool(force_diag)), _ptr(workspace), workspace.numel(),
                             _stream(stream)))
+    return mask_bits
+
+
+SA_STATIC_SCRATCH_BYTES = 2304 * 1024      # include/scalingattn.h
+
+
+def sa_pack_mask_static(scores, density, mask_bits, force_diag: bool = True, stream=None):
+    """sa_pack_mask with the library's fixed scratch array as its workspace: allocates nothing (the
+    caller passes the output tensor). Raises SAError(SA_ERR_WORKSPACE) beyond SA_STATIC_SCRATCH_BYTES."""
+    lib = load_library()
+    assert scores.dtype == torch.float32 and scores.is_contiguous() and scores.dim() == 3
+    assert density.dtype == torch.float32 and density.is_contiguous()
+    H, NQB, NKB = scores.shape
+    assert density.shape == (H,)
+    assert mask_bits.dtype == torch.int32 and mask_bits.is_contiguous()
+    assert tuple(mask_bits.shape) == (H, NQB, (NKB + 31) // 32)
+    _check(lib.sa_pack_mask_static(_ptr(scores), _ptr(density), _ptr(mask_bits), H, NQB, NKB,
+                                   int(bool(force_diag)), _stream(stream)))
     return mask_bits
 
 

@@ -214,6 +214,37 @@ sa_status sa_pack_mask(const float* scores, const float* density, uint32_t* mask
   return SA_OK;
 }
 
+sa_status sa_pack_mask_static(const float* scores, const float* density, uint32_t* mask_bits, int H,
+                              int NQB, int NKB, int force_diag, void* stream) {
+  g_last_launches = 0;
+  if (!scores || !density || !mask_bits)
+    return fail(SA_ERR_INVALID_ARG, "sa_pack_mask_static: null pointer");
+  if (H <= 0 || NQB <= 0 || NKB <= 0)
+    return fail(SA_ERR_INVALID_ARG, "sa_pack_mask_static: sizes must be positive (H=%d NQB=%d NKB=%d)", H,
+                NQB, NKB);
+  if (static_cast<long long>(NQB) * NKB > 0x7FFFFFFFLL)
+    return fail(SA_ERR_UNSUPPORTED, "sa_pack_mask_static: NQB*NKB exceeds 2^31-1");
+  if (!aligned16(scores) || !aligned16(mask_bits))
+    return fail(SA_ERR_INVALID_ARG, "sa_pack_mask_static: pointers must be 16-byte aligned");
+  const size_t need = sa::pack_mask_workspace_bytes(H, NQB, NKB);
+  if (need > static_cast<size_t>(SA_STATIC_SCRATCH_BYTES))
+    return fail(SA_ERR_WORKSPACE,
+                "sa_pack_mask_static: H=%d NQB=%d NKB=%d needs %zu B of scratch, the library's fixed array "
+                "holds %zu B (use sa_pack_mask with a workspace of your own)",
+                H, NQB, NKB, need, static_cast<size_t>(SA_STATIC_SCRATCH_BYTES));
+  sa_status s = check_device();
+  if (s != SA_OK) return s;
+  void* scratch = nullptr;
+  size_t scratch_bytes = 0;
+  cudaError_t e = sa::static_scratch(&scratch, &scratch_bytes);      // device address, looked up once per device
+  if (e != cudaSuccess) return cuda_fail(e, "sa_pack_mask_static: cudaGetSymbolAddress(static scratch)");
+  e = sa::launch_pack_mask(scores, density, mask_bits, H, NQB, NKB, force_diag ? 1 : 0, scratch,
+                           static_cast<cudaStream_t>(stream));
+  if (e != cudaSuccess) return cuda_fail(e, "sa_pack_mask_static launch");
+  g_last_launches = sa::kPackMaskLaunches;
+  return SA_OK;
+}
+
 sa_status sa_mask_from_threshold(const float* tmap, const float* p_star, uint32_t* mask_bits, int H,
                                  int nbq, int nbk, int NQB, int NKB, int force_diag, void* stream) {
   g_last_launches = 0;

@@ -119,6 +119,8 @@ FwdWorkspace carve_fwd_workspace(void* ws, int B, int H, int NQB, int W, TailPla
 enum SmemKernel { kSmemFwdTcgen05 = 0, kSmemFwdTcgen05Lean, kSmemFwdTcgen05Log, kSmemSigTcgen05, kSmemScheduleItems, kSmemFwdMmaSync64,
                   kSmemFwdMmaSync128, kSmemMaskFromThreshold, kNumSmemKernels };
 cudaError_t device_sm_count(int* n_sm);
+// static_scratch.cu: device address and size of the library's fixed scratch array on the current device
+cudaError_t static_scratch(void** ptr, size_t* bytes);
 cudaError_t ensure_dynamic_smem(SmemKernel id, const void* func, int bytes);
 
 // Programmatic dependent launch: the kernel may be scheduled while its predecessor on the stream is
