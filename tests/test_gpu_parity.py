@@ -1058,6 +1058,51 @@ def test_last_round_rows_in_parts_match_oracle(sa, H, N, n_valid, density):
 
 
 
+def test_random_shapes_default_path_against_the_mma_sync_kernel(sa):
+    # Seeded random (B, H, N, mask family, density, ragged tail): whatever work items the default call
+    # picks for the shape -- split items, pairs, the last round in parts, the lean or the full kernel
+    # build -- against the independent mma.sync kernel (variant 1: one CTA per query block, exact
+    # running max) on every row. Both round the same softmax to bf16, so an element may differ by one
+    # bf16 spacing of its value plus the 4e-3 the accumulation orders explain;
+    # run to run the default path gives the same bits. (The oracle comparison proper is above: this
+    # one is cheap enough to cover many shapes.)
+    rng = np.random.default_rng(20261105)
+    seen_launches = set()
+    for case in range(28):
+        nb = int(rng.choice([8, 16, 33, 64, 75, 100, 128, 150, 200, 256]))
+        N = nb * 128
+        H = int(rng.integers(1, max(2, min(24, 3000 // nb)) + 1))
+        B = int(rng.choice([1, 1, 1, 2]))
+        dens = float(rng.choice([1.0, 0.8, 0.5, 0.3, 0.1, 0.03]))
+        kind = int(rng.integers(0, 3))
+        n_valid = N - int(rng.choice([0, 0, 1, 77, 127]))
+        g = torch.Generator().manual_seed(int(rng.integers(1 << 30)))
+        q, k, v = [torch.randn((B, H, N, 128), generator=g).to(torch.bfloat16) for _ in range(3)]
+        idx = np.arange(nb)
+        if kind == 0:                                             # i.i.d.
+            m = rng.random((H, nb, nb)) < dens
+        elif kind == 1:                                           # a few dense rows, the rest sparse
+            m = rng.random((H, nb, nb)) < 0.05
+            m[:, rng.random(nb) < 0.1, :] = True
+        else:                                                     # band + a sink column
+            m = np.broadcast_to(np.abs(idx[:, None] - idx[None, :]) <= max(1, int(dens * nb / 2)),
+                                (H, nb, nb)).copy()
+            m[:, :, 0] = True
+        m[:, idx, idx] = True
+        bits = oracle.pack_bool(m)
+        o0, l0 = run_fwd(sa, q, k, v, bits, 128, 0.0884, n_valid=n_valid, variant=0)
+        seen_launches.add(sa.sa_last_launch_count())
+        o0b, l0b = run_fwd(sa, q, k, v, bits, 128, 0.0884, n_valid=n_valid, variant=0)
+        o1, l1 = run_fwd(sa, q, k, v, bits, 128, 0.0884, n_valid=n_valid, variant=1)
+        what = (case, B, H, nb, kind, dens, n_valid)
+        assert torch.equal(o0, o0b) and torch.equal(l0, l0b), what
+        ref = o1.float()
+        spacing = torch.exp2(torch.floor(torch.log2(ref.abs().clamp_min(1e-30))) - 7)
+        assert ((o0.float() - ref).abs() - spacing).max().item() <= 4e-3, what
+        assert (l0 - l1).abs().max().item() <= 1e-4, what
+    assert seen_launches >= {3, 4}                                # with and without the merge kernel
+
+
 def test_cuda_library_is_the_path(sa):
     # the kernels really ran: launch count reported by the library, and the .so is mapped
     cfg = inputs.C1
