@@ -39,6 +39,8 @@ UNIT = "TFLOP/s"
 # workload, from the `ncu --set full` capture summarised in profiles/ (None until captured).
 NCU_TRAFFIC_BYTES = {"C4": 3335543864}   # dram__bytes_read.sum + dram__bytes_write.sum, one launch
 NCU_TRAFFIC_SOURCE = {"C4": "profiles/r2_fwd_tcgen05_c4_full.md"}
+# l1tex__m_xbar2l1tex_read_bytes.sum of the same launch: what the SMs drew from L2 (K/V/Q tiles)
+NCU_L2_FILL_BYTES = {"C4": 132.2e9}
 
 
 # ------------------------------------------------------------------ pure helpers (CPU-testable)
@@ -654,6 +656,18 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> int:
     west = None
     if rank == 0 and not args.no_west:
         west = run_west_offline(sa, dev, stream, peaks, log)
+    # the L2 -> shared-memory fill rate the SMs can draw (secondary bound of the attention kernel:
+    # its K/V tiles come from L2), measured with bulk copies of 32 KB on every SM (0.3 s)
+    l2_fill = None
+    if rank == 0 and not args.no_west:
+        gbs, n_l = sa.sa_debug_l2_fill_rate(40, 0.3, device=dev, stream=stream)
+        fill = NCU_L2_FILL_BYTES.get(args.workload)
+        l2_fill = {"measured_gbs": round(gbs, 1), "buffer_mb": 40, "launches": n_l,
+                   "kind": "sa_debug_l2_fill_rate: six 32 KB bulk copies in flight per SM, L2-resident buffer",
+                   "attention_kernel_draw_gbs": None if fill is None else round(fill / (kernel_ms_avg * 1e-3) / 1e9, 1),
+                   "attention_kernel_draw_source": None if fill is None else NCU_TRAFFIC_SOURCE.get(args.workload)}
+        log(f"[bench] L2 -> SM fill rate: {gbs:.0f} GB/s measured; the attention kernel draws "
+            f"{l2_fill['attention_kernel_draw_gbs']} GB/s")
 
     dense_lib = None
     if rank == 0 and args.dense_library:
@@ -801,6 +815,7 @@ def run_ours(args, rank: int, local_rank: int, world: int) -> int:
             "density_sweep": sweep,
             "seqlen_grid": seq_grid,
             "west_offline": west,
+            "l2_fill": l2_fill,
             "dense_library_context": dense_lib,
         }
         print(json.dumps(line), flush=True)

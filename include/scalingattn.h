@@ -271,6 +271,15 @@ SA_API sa_status sa_fwd_softmax_path_counts(const void* workspace, long long* fi
  * Call it in a loop for a sustained-load figure. */
 SA_API sa_status sa_debug_ex2_rate(int iters, float* sink, float* ms_host, double* n_exp_host, void* stream);
 
+/* Measurement hook for the secondary bound of the attention kernel on masks whose work items share no
+ * key blocks (every (query tile, key block) unit then needs 64 KB of K and V from L2): one CTA per SM
+ * keeps six 32 KB bulk copies global -> shared memory in flight, `iters` copies per SM, walking `buf`
+ * (device, 16 B aligned, `buf_bytes` >= 32 KB; a buffer that fits L2 is served from L2 after the first
+ * pass). Runs one launch on `stream`, waits for it, returns its milliseconds in *ms_host and the bytes it
+ * moved in *bytes_host (host pointers). */
+SA_API sa_status sa_debug_l2_fill_rate(const void* buf, size_t buf_bytes, int iters, float* ms_host,
+                                       double* bytes_host, void* stream);
+
 /* Debug hook: sa_block_sparse_attn_fwd_ex on a build of the (128,128,128) tcgen05 kernel that also
  * records its walk, so that the union walk of a work item (Alg. 2 re-expressed over the OR of two
  * bit-rows), the numbering of (tile, key block) units and the 64-word window reload can be checked

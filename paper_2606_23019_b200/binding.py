@@ -74,6 +74,8 @@ def load_library() -> C.CDLL:
     lib.sa_fwd_softmax_path_counts.argtypes = [vp, vp, vp, vp]
     lib.sa_debug_tail_plan.restype = ip
     lib.sa_debug_tail_plan.argtypes = [ip, ip, ip, ip, ip, ip, vp, vp]
+    lib.sa_debug_l2_fill_rate.restype = ip
+    lib.sa_debug_l2_fill_rate.argtypes = [vp, sz, ip, vp, vp, vp]
     lib.sa_debug_ex2_rate.restype = ip
     lib.sa_debug_ex2_rate.argtypes = [ip, vp, vp, vp, vp]
     lib.sa_debug_fwd_walk_log_bytes.restype = sz
@@ -339,6 +341,29 @@ def sa_debug_tail_plan(B: int, H: int, N: int, Bq: int, Bk: int, n_sm: int):
     rem, parts = C.c_int(0), C.c_int(0)
     _check(load_library().sa_debug_tail_plan(B, H, N, Bq, Bk, n_sm, C.addressof(rem), C.addressof(parts)))
     return rem.value, parts.value
+
+
+def sa_debug_l2_fill_rate(buf_mb: int = 40, seconds: float = 0.3, iters: int = 4096, device=None, stream=None):
+    """Measured L2 -> shared-memory fill rate in GB/s (every SM streaming 32 KB tiles of a `buf_mb` MB
+    buffer with bulk copies), sustained over about `seconds`. Returns (GB/s, launches)."""
+    import time
+    lib = load_library()
+    device = torch.device("cuda", torch.cuda.current_device()) if device is None else device
+    buf = torch.zeros(buf_mb << 20, dtype=torch.uint8, device=device)
+    ms, nbytes = C.c_float(0.0), C.c_double(0.0)
+    tot_ms = tot_b = 0.0
+    n = 0
+    t0 = time.time()
+    while True:
+        _check(lib.sa_debug_l2_fill_rate(_ptr(buf), buf.numel(), int(iters), C.addressof(ms), C.addressof(nbytes),
+                                         _stream(stream)))
+        n += 1
+        if n > 1:                                  # the first launch fills L2
+            tot_ms += ms.value
+            tot_b += nbytes.value
+        if time.time() - t0 > seconds and n >= 3:
+            break
+    return tot_b / (tot_ms * 1e-3) / 1e9, n
 
 
 def sa_debug_ex2_rate(seconds: float = 0.5, iters: int = 4096, device=None, stream=None):

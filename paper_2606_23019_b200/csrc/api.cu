@@ -756,6 +756,32 @@ sa_status sa_debug_ex2_rate(int iters, float* sink, float* ms_host, double* n_ex
   return SA_OK;
 }
 
+sa_status sa_debug_l2_fill_rate(const void* buf, size_t buf_bytes, int iters, float* ms_host,
+                                double* bytes_host, void* stream) {
+  if (!buf || !ms_host || !bytes_host || iters <= 0 || buf_bytes < 32768 || !aligned16(buf))
+    return fail(SA_ERR_INVALID_ARG, "sa_debug_l2_fill_rate: bad arguments");
+  sa_status s = check_device();
+  if (s != SA_OK) return s;
+  int n_sm = 0;
+  cudaError_t e = sa::device_sm_count(&n_sm);
+  if (e != cudaSuccess) return cuda_fail(e, "device query");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  cudaEvent_t a = nullptr, b = nullptr;
+  if ((e = cudaEventCreate(&a)) != cudaSuccess || (e = cudaEventCreate(&b)) != cudaSuccess) {
+    if (a) cudaEventDestroy(a);
+    return cuda_fail(e, "cudaEventCreate");
+  }
+  e = cudaEventRecord(a, st);
+  if (e == cudaSuccess) e = sa::launch_l2_fill(buf, buf_bytes, iters, n_sm, st, bytes_host);
+  if (e == cudaSuccess) e = cudaEventRecord(b, st);
+  if (e == cudaSuccess) e = cudaEventSynchronize(b);
+  if (e == cudaSuccess) e = cudaEventElapsedTime(ms_host, a, b);
+  cudaEventDestroy(a);
+  cudaEventDestroy(b);
+  if (e != cudaSuccess) return cuda_fail(e, "sa_debug_l2_fill_rate");
+  return SA_OK;
+}
+
 sa_status sa_set_fwd_variant(int variant) {
   if (variant < 0 || variant > 3)
     return fail(SA_ERR_INVALID_ARG, "sa_set_fwd_variant: variant %d not in {0,1,2,3}", variant);

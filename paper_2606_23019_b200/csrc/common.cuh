@@ -117,7 +117,7 @@ FwdWorkspace carve_fwd_workspace(void* ws, int B, int H, int NQB, int W, TailPla
 // per-device state (device.cu): SM count of the current device; dynamic shared-memory opt-in of a
 // kernel, set once per (device, kernel)
 enum SmemKernel { kSmemFwdTcgen05 = 0, kSmemFwdTcgen05Lean, kSmemFwdTcgen05Log, kSmemSigTcgen05, kSmemScheduleItems, kSmemFwdMmaSync64,
-                  kSmemFwdMmaSync128, kSmemMaskFromThreshold, kNumSmemKernels };
+                  kSmemFwdMmaSync128, kSmemMaskFromThreshold, kSmemL2Fill, kNumSmemKernels };
 cudaError_t device_sm_count(int* n_sm);
 // static_scratch.cu: device address and size of the library's fixed scratch array on the current device
 cudaError_t static_scratch(void** ptr, size_t* bytes);
@@ -175,6 +175,8 @@ cudaError_t launch_fidelity(const float* lse_dense, const float* lse_sparse, con
                             int n_rows, int BH, int N, float* fidelity, float* per_row,
                             cudaStream_t st);
 cudaError_t launch_ex2_rate(int iters, float* sink, int n_sm, cudaStream_t st, double* n_exp);
+cudaError_t launch_l2_fill(const void* buf, size_t buf_bytes, int iters, int n_sm, cudaStream_t st,
+                           double* bytes_moved);
 cudaError_t launch_enumerate(const uint32_t* mask_bits, int H, int NQB, int NKB, int32_t* idx,
                              int32_t* cnt, cudaStream_t st);
 
