@@ -37,7 +37,7 @@ UNIT = "TFLOP/s"
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the attention kernel at the bench
 # workload, from the `ncu --set full` capture summarised in profiles/ (None until captured).
-NCU_TRAFFIC_BYTES = {"C4": 3335543864}   # dram__bytes_read.sum + dram__bytes_write.sum, one launch
+NCU_TRAFFIC_BYTES = {"C4": 3324382176}   # dram__bytes_read.sum + dram__bytes_write.sum, one launch
 NCU_TRAFFIC_SOURCE = {"C4": "profiles/r2_fwd_tcgen05_c4_full.md"}
 # l1tex__m_xbar2l1tex_read_bytes.sum of the same launch: what the SMs drew from L2 (K/V/Q tiles)
 NCU_L2_FILL_BYTES = {"C4": 132.2e9}
