@@ -616,8 +616,8 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
     mbar_wait(smem_u32(&ctl->q_full), qf_phase, 24);
     SA_TR(6);
     qf_phase ^= 1u;
-    bound = 0.f;
-    if (exists) {
+    bound = INFINITY;                    // no bound (sparse group / small problem): exact running max,
+    if (exists && p.kmax2 != nullptr && kmax2 >= 0.f) {      // and the row norms are not needed
       const uint32_t qrow = smem_base + kOffQ + (it.split() ? 0 : t) * kTileBytes + row * 128;
       float qn2 = 0.f;
 #pragma unroll
@@ -634,7 +634,7 @@ __device__ void softmax_wg(const FwdParams& p, Ctl* ctl, uint32_t smem_base, uin
           qn2 = fmaf(hi, hi, qn2);
         }
       }
-      bound = (p.kmax2 && kmax2 >= 0.f) ? c * sqrtf(qn2) * sqrtf(kmax2) : INFINITY;   // no bound: exact max
+      bound = c * sqrtf(qn2) * sqrtf(kmax2);
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(smem_u32(&ctl->q_empty));   // this warp is done with the Q tiles
