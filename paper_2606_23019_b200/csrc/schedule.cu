@@ -102,6 +102,7 @@ FwdWorkspace carve_fwd_workspace(void* ws, int B, int H, int NQB, int W, TailPla
 namespace {
 
 constexpr int kSortThreads = 1024;
+constexpr int kMinSingleBlocks = 3;       // rows of a tail pair that run as single-row items hold at least this many
 constexpr int kMaxTail = 128;             // rows-in-parts of one (b,h) group (fwd_tail_plan: <= n_sm per launch)
 constexpr uint32_t kIdxBits = 14, kIdxMask = (1u << kIdxBits) - 1u;       // rows / slots < 16384
 
@@ -392,6 +393,10 @@ schedule_items_kernel(const uint32_t* __restrict__ mask_bits, int H, int NQB, in
       }
       done += chunk;
     }
+    // too short for parts, but a real pair: its two rows become two SINGLE-ROW items (ub = 0xFFFF, the
+    // kernel's second tile idle) at the end of the order -- about 0.6 of the pair's time each, which
+    // is what the partly filled last round then takes (np = -2 marks it)
+    if (np == 1 && b != 0xFFFF && b != a && min(s_pop[a], s_pop[b]) >= kMinSingleBlocks) np = -2;
     if (lane == 0) s_np[k] = np;
   }
   __syncthreads();
@@ -404,9 +409,9 @@ schedule_items_kernel(const uint32_t* __restrict__ mask_bits, int H, int NQB, in
       if (s_np[k] == 1) s_at[k] = at++;
     s_main_end = at;
     for (int k = 0; k < n_tail; ++k)
-      if (s_np[k] > 1) {
+      if (s_np[k] != 1) {
         s_at[k] = at;
-        at += s_np[k];
+        at += abs(s_np[k]);
       }
     s_at[n_tail] = at;
   }
@@ -416,6 +421,15 @@ schedule_items_kernel(const uint32_t* __restrict__ mask_bits, int H, int NQB, in
     const int s = static_cast<int>(kIdxMask - (key & kIdxMask));
     const int rows_ab = s_a[s] | (s_b[s] << 16);
     const int np = s_np[k], slot0 = (t0 + k) * plan_parts;
+    if (np == -2) {
+      if (lane < 2) {
+        const int u = lane == 0 ? (rows_ab & 0xFFFF) : ((rows_ab >> 16) & 0xFFFF);
+        local_items[static_cast<size_t>(bh) * NQB + s_at[k] + lane] =
+            make_int4(s_pop[u], u | (0xFFFF << 16), -1, 0);
+      }
+      if (lane == 0) tasks[t0 + k] = make_int4(-1, rows_ab, 1, slot0);
+      continue;
+    }
     if (lane < np)
       local_items[static_cast<size_t>(bh) * NQB + s_at[k] + lane] =
           make_int4(static_cast<int>(key >> kIdxBits) - 1, rows_ab, np > 1 ? slot0 + lane : -1, 0);
